@@ -1,0 +1,131 @@
+/* bs.h -- C ABI of libbs: Pauli-sum operator x sector state-vector multiplication on one B200.
+ *
+ * Implements the operator-state multiplication path of arxiv/paper_2606_28952 ("BinSim")
+ * section 2.4-2.5: a Pauli sum held in binary symplectic form
+ * (x mask, z mask, complex coefficient per string; Eq. 12-18) is canonically
+ * reduced, grouped by X mask (Eq. 24) and applied to a state
+ * vector restricted to an (N_alpha, N_beta) sector (Eq. 25, 28, 38) by
+ * target-configuration gathers (Eq. 27).
+ *
+ * Conventions (DESIGN.md "Readings" U1-U5):
+ *   - qubit k = bit k of the 64-bit masks; a string is (x) over k of {I,X,Y,Z} with
+ *     (x_k, z_k) = (0,0) I, (1,0) X, (1,1) Y, (0,1) Z                    (Eq. 8).
+ *   - coefficients are those of the TRUE Pauli string (not of the XZ-ordered product).
+ *   - matrix element: <t| c P |s> = c * (-i)^{ny} * (-1)^{popc(z & t)}, t = s ^ x,
+ *     ny = popc(x & z).  The library stores the target-form weight w = c * (-i)^{ny}.
+ *   - blocked spin ordering: alpha spin-orbital p = qubit p, beta spin-orbital p = qubit n_orb+p;
+ *     bit = 1 means occupied.
+ *   - sector vector layout: index(t) = rank_alpha(t_a) * D_beta + rank_beta(t_b), where
+ *     t_a = t & (2^n_orb - 1), t_b = t >> n_orb, and rank_s is the combinatorial-number-system
+ *     rank (= position among all n_orb-bit words of popcount N_s in increasing numeric order).
+ *     Full-space mode (n_alpha = n_beta = -1): index(t) = t.
+ *   - all state vectors are complex128, interleaved (re, im), 16-byte aligned DEVICE pointers,
+ *     owned by the caller; the library never retains them past the call.
+ *
+ * Pointers are marked [host] or [device].  Every call returns a bs_status (0 = OK, negative =
+ * error, outputs untouched on error) and never throws across the ABI; bs_last_error() gives a
+ * thread-local message.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default
+ * stream); kernels are enqueued on it and the call returns without synchronising unless stated.
+ * There is NO CPU fallback: without a CUDA device every compute entry point returns BS_ERR_CUDA.
+ */
+#ifndef BS_H_
+#define BS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bs_op*     bs_op_t;     /* grouped Pauli sum, device resident, library owned */
+typedef struct bs_sector* bs_sector_t; /* sector tables,     device resident, library owned */
+
+typedef enum {
+    BS_OK = 0,
+    BS_ERR_ARG = -1,           /* bad argument (null pointer, size, alignment, n_qubits > 64 ...)  */
+    BS_ERR_ALLOC = -2,         /* host or device allocation failed                                */
+    BS_ERR_CUDA = -3,          /* CUDA runtime error / no device                                  */
+    BS_ERR_MISMATCH = -4,      /* operator and sector disagree on the qubit count                 */
+    BS_ERR_NOT_COMMUTING = -5, /* a rotation generator's strings do not mutually commute          */
+    BS_ERR_LEAVES_SECTOR = -6  /* a rotation generator maps the sector outside itself             */
+} bs_status;
+
+#define BS_MODE_CANONICAL 0
+#define BS_MODE_SEQUENCE  1
+
+/* ---- a1 + a2: canonical reduction and X-mask grouping (Eq. 24).
+ * x, z [host] u64[M]; coeff_reim [host] double[2M] (true-Pauli coefficients c_k).
+ * mode BS_MODE_CANONICAL: sort by key (x major, z minor, unsigned ascending; stable), sum the
+ *   coefficients of equal keys in INPUT order, drop |c| < eps_drop, segment by x.  Runs on the
+ *   device (radix sort, segmented sum, compaction).  seq_offsets must be NULL.
+ * mode BS_MODE_SEQUENCE: strings [seq_offsets[j], seq_offsets[j+1]) (j < n_seq, seq_offsets[0]=0,
+ *   seq_offsets[n_seq]=M) form group j, kept in input order, no merge, no drop; every string of
+ *   a run must carry the same x (else BS_ERR_ARG).  Used for rotation generators,
+ *   whose order matters.
+ * Synchronises the stream before returning (the group count is needed on the host). */
+int bs_group_xmask(const uint64_t* x, const uint64_t* z, const double* coeff_reim, int64_t M,
+                   int n_qubits, double eps_drop, int mode, const int64_t* seq_offsets,
+                   int64_t n_seq, void* cuda_stream, bs_op_t* out);
+int bs_op_info(bs_op_t op, int64_t* n_groups, int64_t* n_terms, int* n_qubits);
+/* Host copies of the device tables; any pointer may be NULL.  xg u64[G] group masks; offs
+ * i64[G+1] string offsets; z u64[M]; c_reim double[2M] true-Pauli coefficients; w_reim
+ * double[2M] target-form weights w_k = c_k (-i)^{ny_k}. */
+int bs_op_export(bs_op_t op, uint64_t* xg, int64_t* offs, uint64_t* z, double* c_reim, double* w_reim);
+int bs_op_destroy(bs_op_t op);
+
+/* ---- a3: sector tables.  n_alpha = n_beta = -1: full 2^n space and
+ * n_orb then means n_qubits.  Sector mode needs n_orb <= 32, 0 <= n_alpha, n_beta <= n_orb. */
+int bs_sector_build(int n_orb, int n_alpha, int n_beta, void* cuda_stream, bs_sector_t* out);
+int bs_sector_info(bs_sector_t s, int64_t* dim, int64_t* dim_alpha, int64_t* dim_beta);
+/* alpha_strings [host] u64[dim_alpha], beta_strings [host] u64[dim_beta]: unrank tables. */
+int bs_sector_export(bs_sector_t s, uint64_t* alpha_strings, uint64_t* beta_strings);
+/* configs [host] u64[n] -> index_out [host] i64[n] (-1 outside the sector); ranks on the device
+ * with the same lookup tables the apply kernels use.  Synchronises. */
+int bs_sector_rank(bs_sector_t s, const uint64_t* configs, int64_t n, int64_t* index_out);
+int bs_sector_destroy(bs_sector_t s);
+
+/* ---- a4: out = P_sector H P_sector psi  (Eq. 27).  psi_in, psi_out [device]
+ * complex128[dim], distinct buffers.  The first call for a given (op, sector) pair builds and
+ * caches sector-specific device tables (synchronises once); later calls only launch. */
+int bs_apply(bs_op_t op, bs_sector_t s, const void* psi_in, void* psi_out, void* cuda_stream);
+/* Same, for alpha rows [row_lo, row_hi) only (full-space mode: index range): writes
+ * psi_out[row_lo*D_beta .. row_hi*D_beta) and nothing else.  This is the multi-GPU shard unit
+ * (targets are independent). */
+int bs_apply_rows(bs_op_t op, bs_sector_t s, const void* psi_in, void* psi_out, int64_t row_lo,
+                  int64_t row_hi, void* cuda_stream);
+/* out = alpha * (H psi_in) + beta * psi_in, and if acc != NULL additionally acc += out, fused into
+ * the apply epilogue (the Taylor recurrence of PAPER.md:74-83, Eq. 6-7).  alpha, beta [host]
+ * double[2] complex; acc [device] complex128[dim] or NULL. */
+int bs_apply_axpby(bs_op_t op, bs_sector_t s, const void* psi_in, void* psi_out,
+                   const double alpha_reim[2], const double beta_reim[2], void* acc,
+                   void* cuda_stream);
+
+/* ---- a5: <psi|H|psi> (Eq. 5), fused gather + dot, H psi is never stored.
+ * result_reim [host] double[2]; deterministic two-stage reduction.  Synchronises the stream. */
+int bs_expect(bs_op_t op, bs_sector_t s, const void* psi, double result_reim[2], void* cuda_stream);
+/* <a|b> = sum conj(a_i) b_i over dim amplitudes, same deterministic reduction.  Synchronises. */
+int bs_vdot(bs_sector_t s, const void* a, const void* b, double result_reim[2], void* cuda_stream);
+
+/* ---- a6: psi <- exp(theta_j A_j) psi for j = 0..n_rot-1 in order, A_j = group j of a
+ * BS_MODE_SEQUENCE operator: anti-Hermitian (every c_k purely imaginary), one x != 0, mutually
+ * commuting strings (Eq. 39).  thetas [host] double[n_rot], n_rot must
+ * equal the operator's group count.  In place on disjoint pairs {t, t^x}.  Returns
+ * BS_ERR_NOT_COMMUTING / BS_ERR_LEAVES_SECTOR instead of applying a non-unitary map.
+ * Synchronises the stream (the leak flag is read back). */
+int bs_apply_pauli_rotations(bs_op_t generators, bs_sector_t s, const double* thetas,
+                             int64_t n_rot, void* psi_inout, void* cuda_stream);
+
+/* ---- a7: one step psi <- e^{-i E_s dt} sum_{k<=order} (-i dt)^k/k! (H - E_s)^k psi
+ * (Eq. 6-7; reading U9).  work [device] complex128[2*dim] scratch. */
+int bs_taylor_step(bs_op_t op, bs_sector_t s, void* psi_inout, void* work, double dt, int order,
+                   double e_shift, void* cuda_stream);
+
+/* number of kernels this library has launched in this process (for bench.py's gpu_launches) */
+int64_t bs_launch_count(void);
+const char* bs_last_error(void);
+const char* bs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BS_H_ */

@@ -1,0 +1,123 @@
+// Internal declarations of libbs (not part of the ABI; the ABI is include/bs.h).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "bs.h"
+
+using u64 = uint64_t;
+using u32 = uint32_t;
+using i64 = int64_t;
+
+// ---- errors ---------------------------------------------------------------------------------
+void bs_set_error(const char* fmt, ...);
+extern std::atomic<int64_t> g_bs_launches;
+#define BS_COUNT_LAUNCH(n) (g_bs_launches.fetch_add((n), std::memory_order_relaxed))
+
+#define BS_CUDA(call)                                                                       \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            bs_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? BS_ERR_ALLOC : BS_ERR_CUDA;         \
+        }                                                                                   \
+    } while (0)
+
+#define BS_REQUIRE(cond, status, ...)   \
+    do {                                \
+        if (!(cond)) {                  \
+            bs_set_error(__VA_ARGS__);  \
+            return (status);            \
+        }                               \
+    } while (0)
+
+// RAII device buffer (library-owned tables only; never state vectors).
+template <class T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t n = 0;
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete;
+    DevBuf& operator=(const DevBuf&) = delete;
+    ~DevBuf() { release(); }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+    // allocates n_ elements plus `pad` bytes of slack (bulk copies round sizes up to 16 B)
+    cudaError_t alloc(size_t n_, size_t pad = 64) {
+        release();
+        n = n_;
+        return cudaMalloc((void**)&p, n_ * sizeof(T) + pad);
+    }
+    cudaError_t upload(const std::vector<T>& h, cudaStream_t st) {
+        cudaError_t e = alloc(h.size());
+        if (e != cudaSuccess || h.empty()) return e;
+        return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+    }
+};
+
+// ---- operator -------------------------------------------------------------------------------
+struct bs_op {
+    u64 id;        // unique handle id (plan cache key)
+    int n_qubits;
+    int mode;
+    i64 G, M;      // groups, strings
+    // host mirrors of the canonical tables (used by bs_op_export and by the plan builder)
+    std::vector<u64> h_xg, h_z;
+    std::vector<i64> h_offs;
+    std::vector<double> h_c, h_w;  // 2*M each
+    // device tables (SURVEY 8(a) a2 layout)
+    DevBuf<u64> d_xg, d_z;
+    DevBuf<i64> d_offs;
+    DevBuf<double2> d_w;
+};
+
+// ---- sector ---------------------------------------------------------------------------------
+// Device view of one spin's rank/unrank tables.  rank(w) = lo[w & mask_lo] +
+// hi[popc(w & mask_lo) << bits_hi | (w >> bits_lo)] for words of the right popcount.
+struct SpinTab {
+    const u32* str;  // unrank: D words, increasing
+    const u32* lo;   // 2^bits_lo entries
+    const u32* hi;   // (N+1) * 2^bits_hi entries
+    int bits_lo, bits_hi, N;
+    u32 mask_lo;
+    i64 D;
+};
+
+struct bs_sector {
+    u64 id;
+    bool full;
+    int n_orb, n_alpha, n_beta, n_qubits;
+    i64 D, Da, Db;
+    std::vector<u64> h_sa, h_sb;
+    DevBuf<u32> d_sa, d_sb, d_lo_a, d_hi_a, d_lo_b, d_hi_b;
+    SpinTab ta, tb;
+    // scratch for deterministic reductions (partials of bs_expect / bs_vdot) and flags
+    DevBuf<double2> d_partials;
+    DevBuf<double2> d_result;
+    DevBuf<int> d_flag;
+};
+
+__device__ __forceinline__ u32 spin_rank(const SpinTab& t, u32 w) {
+    u32 l = w & t.mask_lo;
+    u32 r = __ldg(t.lo + l);
+    if (t.bits_hi > 0) r += __ldg(t.hi + ((u32)__popc(l) << t.bits_hi | (w >> t.bits_lo)));
+    return r;
+}
+
+// ---- plan: sector-specific tables of one (operator, sector) pair -------------------------------
+struct bs_plan;
+int bs_plan_get(bs_op* op, bs_sector* s, cudaStream_t st, bs_plan** out);
+void bs_plan_purge(u64 op_id, u64 sector_id);
+
+u64 bs_next_id();
