@@ -111,7 +111,8 @@ int bs_vdot(bs_sector_t s, const void* a, const void* b, double result_reim[2], 
  * commuting strings (Eq. 39).  thetas [host] double[n_rot], n_rot must
  * equal the operator's group count.  In place on disjoint pairs {t, t^x}.  Returns
  * BS_ERR_NOT_COMMUTING / BS_ERR_LEAVES_SECTOR instead of applying a non-unitary map.
- * Synchronises the stream (the leak flag is read back). */
+ * The first call for a (generators, sector) pair runs a read-only leak check and synchronises; later
+ * calls only enqueue n_rot launches. */
 int bs_apply_pauli_rotations(bs_op_t generators, bs_sector_t s, const double* thetas,
                              int64_t n_rot, void* psi_inout, void* cuda_stream);
 

@@ -80,6 +80,7 @@ struct bs_op {
     DevBuf<u64> d_xg, d_z;
     DevBuf<i64> d_offs;
     DevBuf<double2> d_w;
+    std::vector<u64> validated_sectors;  // sector ids this generator list was leak-checked against
 };
 
 // ---- sector ---------------------------------------------------------------------------------

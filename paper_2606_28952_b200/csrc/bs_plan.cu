@@ -1,0 +1,212 @@
+// Plan builder: turns the canonical group tables of an operator (a2) into the sector-specific
+// layout the apply kernels stream (spin-split masks, z-reduction, per-row valid alpha masks).
+// PAPER.md:227-231 (Eq. 28: X_g = (X_ga, X_gb), Z_k = (Z_ka, Z_kb)), PAPER.md:247 (factorised phase).
+#include <cub/cub.cuh>
+
+#include <algorithm>
+
+#include "bs_plan.cuh"
+
+namespace {
+
+std::mutex g_plan_mu;
+std::map<std::pair<u64, u64>, bs_plan*> g_plans;
+
+// count / fill the valid alpha masks of every target alpha row: mask xa is valid for row string ta
+// iff ta ^ xa has the same popcount, i.e. 2 popc(ta & xa) = popc(xa).  One thread per row walks
+// the masks in ascending order, so the list order (and hence the summation order) is fixed.
+__global__ void k_row_count(SpinTab A, const u32* __restrict__ xa, int n_xa, int* __restrict__ cnt) {
+    i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (r >= A.D) return;
+    u32 ta = A.str[r];
+    int c = 0;
+    for (int i = 0; i < n_xa; ++i) {
+        u32 m = __ldg(xa + i);
+        c += (2 * __popc(ta & m) == __popc(m));
+    }
+    cnt[r] = c;
+}
+
+__global__ void k_row_fill(SpinTab A, const u32* __restrict__ xa, int n_xa, const i64* __restrict__ off,
+                           uint2* __restrict__ ent) {
+    i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (r >= A.D) return;
+    u32 ta = A.str[r];
+    i64 o = off[r];
+    for (int i = 0; i < n_xa; ++i) {
+        u32 m = __ldg(xa + i);
+        if (2 * __popc(ta & m) == __popc(m)) ent[o++] = make_uint2((u32)i, spin_rank(A, ta ^ m));
+    }
+}
+
+struct HostStr {
+    u32 za, zb;
+    double re, im;
+};
+struct HostGroup {
+    u32 xa, xb;
+    std::vector<HostStr> s;
+};
+
+int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
+    const int n = S->n_orb;
+    const u64 mask_a = (n == 64) ? ~u64(0) : ((u64(1) << n) - 1);
+    std::vector<HostGroup> groups;
+    groups.reserve(op->G);
+    bool real_w = true;
+    for (i64 g = 0; g < op->G; ++g) {
+        u64 x = op->h_xg[g];
+        u32 xa = (u32)(x & mask_a), xb = (u32)(x >> n);
+        int pa = __builtin_popcount(xa), pb = __builtin_popcount(xb);
+        if ((pa & 1) || (pb & 1)) continue;  // can never conserve N_alpha / N_beta
+        if (pa / 2 > std::min(S->n_alpha, n - S->n_alpha) || pb / 2 > std::min(S->n_beta, n - S->n_beta)) continue;
+        HostGroup hg;
+        hg.xa = xa;
+        hg.xb = xb;
+        double sga = ((pa / 2) & 1) ? -1.0 : 1.0, sgb = ((pb / 2) & 1) ? -1.0 : 1.0;
+        for (i64 k = op->h_offs[g]; k < op->h_offs[g + 1]; ++k) {
+            u64 z = op->h_z[k];
+            HostStr s{(u32)(z & mask_a), (u32)(z >> n), op->h_w[2 * k], op->h_w[2 * k + 1]};
+            // z-reduction modulo x (exact on valid targets, see bs_plan.cuh)
+            if ((s.za ^ xa) < s.za) { s.za ^= xa; s.re *= sga; s.im *= sga; }
+            if ((s.zb ^ xb) < s.zb) { s.zb ^= xb; s.re *= sgb; s.im *= sgb; }
+            hg.s.push_back(s);
+        }
+        std::stable_sort(hg.s.begin(), hg.s.end(), [](const HostStr& a, const HostStr& b) {
+            return a.zb < b.zb || (a.zb == b.zb && a.za < b.za);
+        });
+        std::vector<HostStr> m;
+        for (auto& s : hg.s) {
+            if (!m.empty() && m.back().za == s.za && m.back().zb == s.zb) {
+                m.back().re += s.re;
+                m.back().im += s.im;
+            } else m.push_back(s);
+        }
+        hg.s.clear();
+        for (auto& s : m)
+            if (s.re != 0.0 || s.im != 0.0) {
+                hg.s.push_back(s);
+                if (s.im != 0.0) real_w = false;
+            }
+        if (!hg.s.empty()) groups.push_back(std::move(hg));
+    }
+    std::stable_sort(groups.begin(), groups.end(), [](const HostGroup& a, const HostGroup& b) {
+        return a.xa < b.xa || (a.xa == b.xa && a.xb < b.xb);
+    });
+    std::vector<u32> xa_list, ga_off;
+    std::vector<uint4> hdr;
+    std::vector<uint2> szab;
+    std::vector<double2> sw;
+    for (size_t g = 0; g < groups.size(); ++g) {
+        if (g == 0 || groups[g].xa != groups[g - 1].xa) {
+            xa_list.push_back(groups[g].xa);
+            ga_off.push_back((u32)g);
+        }
+        hdr.push_back(make_uint4(groups[g].xb, (u32)szab.size(), (u32)groups[g].s.size(),
+                                 (u32)__builtin_popcount(groups[g].xb)));
+        for (auto& s : groups[g].s) {
+            szab.push_back(make_uint2(s.za, s.zb));
+            sw.push_back(make_double2(s.re, s.im));
+        }
+    }
+    ga_off.push_back((u32)groups.size());
+    P->real_w = real_w;
+    P->n_xa = (int)xa_list.size();
+    P->n_groups = (i64)groups.size();
+    P->n_strings = (i64)szab.size();
+    BS_CUDA(P->d_xa.upload(xa_list, st));
+    BS_CUDA(P->d_ga_off.upload(ga_off, st));
+    BS_CUDA(P->d_ghdr.upload(hdr, st));
+    BS_CUDA(P->d_szab.upload(szab, st));
+    BS_CUDA(P->d_sw.upload(sw, st));
+
+    // per-row valid alpha masks
+    const i64 Da = S->Da;
+    DevBuf<int> cnt;
+    DevBuf<i64> cnt64;
+    BS_CUDA(cnt.alloc(Da));
+    BS_CUDA(P->d_row_off.alloc(Da + 1));
+    unsigned nb = (unsigned)((Da + 127) / 128);
+    k_row_count<<<nb, 128, 0, st>>>(S->ta, P->d_xa.p, P->n_xa, cnt.p);
+    std::vector<int> hcnt(Da);
+    BS_CUDA(cudaMemcpyAsync(hcnt.data(), cnt.p, Da * 4, cudaMemcpyDeviceToHost, st));
+    BS_CUDA(cudaStreamSynchronize(st));
+    std::vector<i64> hoff(Da + 1, 0);
+    int mx = 0;
+    for (i64 r = 0; r < Da; ++r) {
+        hoff[r + 1] = hoff[r] + hcnt[r];
+        mx = std::max(mx, hcnt[r]);
+    }
+    P->n_row_ent = hoff[Da];
+    P->max_row_ent = mx;
+    BS_CUDA(cudaMemcpyAsync(P->d_row_off.p, hoff.data(), (Da + 1) * 8, cudaMemcpyHostToDevice, st));
+    BS_CUDA(P->d_row_ent.alloc(P->n_row_ent));
+    k_row_fill<<<nb, 128, 0, st>>>(S->ta, P->d_xa.p, P->n_xa, P->d_row_off.p, P->d_row_ent.p);
+    BS_COUNT_LAUNCH(2);
+    BS_CUDA(cudaGetLastError());
+    BS_CUDA(cudaStreamSynchronize(st));
+    return BS_OK;
+}
+
+int build_full_plan(bs_plan* P, bs_op* op, cudaStream_t st, int max_strings) {
+    // fixed-size chunks over the string stream; a chunk may split a group (the kernel gathers the
+    // source amplitude once per piece, which is linear and therefore exact).  Every group owns at
+    // least one string, so a chunk touches at most max_strings groups.
+    i64 M = op->M, G = op->G;
+    bool real_w = true;
+    for (i64 k = 0; k < M; ++k)
+        if (op->h_w[2 * k + 1] != 0.0) real_w = false;
+    P->real_w = real_w;
+    i64 g = 0;
+    for (i64 s = 0; s < M; s += max_strings) {   // max_strings is even: s0 stays 16-byte aligned
+        i64 e = std::min(M, s + max_strings);
+        while (op->h_offs[g + 1] <= s) ++g;
+        i64 ge = g;
+        while (ge + 1 < G && op->h_offs[ge + 1] < e) ++ge;
+        P->h_chunks.push_back(FullChunk{(int)g, (int)ge, (int)s, (int)e});
+    }
+    P->n_chunks = (int)P->h_chunks.size();
+    BS_CUDA(P->d_chunks.upload(P->h_chunks, st));
+    BS_CUDA(cudaStreamSynchronize(st));
+    return BS_OK;
+}
+
+}  // namespace
+
+// full-space staging capacities (must match bs_apply.cu)
+extern const int kFullChunkStrings = 512;
+
+int bs_plan_get(bs_op* op, bs_sector* s, cudaStream_t st, bs_plan** out) {
+    std::lock_guard<std::mutex> lk(g_plan_mu);
+    auto key = std::make_pair(op->id, s->id);
+    auto it = g_plans.find(key);
+    if (it != g_plans.end()) {
+        *out = it->second;
+        return BS_OK;
+    }
+    BS_REQUIRE(op->n_qubits == s->n_qubits, BS_ERR_MISMATCH, "operator has %d qubits, sector has %d", op->n_qubits,
+               s->n_qubits);
+    bs_plan* P = new (std::nothrow) bs_plan;
+    BS_REQUIRE(P, BS_ERR_ALLOC, "plan allocation failed");
+    P->op_id = op->id;
+    P->sector_id = s->id;
+    P->full = s->full;
+    int rc = s->full ? build_full_plan(P, op, st, kFullChunkStrings) : build_sector_plan(P, op, s, st);
+    if (rc != BS_OK) {
+        delete P;
+        return rc;
+    }
+    g_plans[key] = P;
+    *out = P;
+    return BS_OK;
+}
+
+void bs_plan_purge(u64 op_id, u64 sector_id) {
+    std::lock_guard<std::mutex> lk(g_plan_mu);
+    for (auto it = g_plans.begin(); it != g_plans.end();) {
+        if ((op_id && it->first.first == op_id) || (sector_id && it->first.second == sector_id)) {
+            delete it->second;
+            it = g_plans.erase(it);
+        } else ++it;
+    }
+}
