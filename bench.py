@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- H|psi> applies/s (complex128) and achieved HBM GB/s vs the measured B200 peak.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+                    [--per-config q12,q24,...|none]
+
+Headline workload (config.workload): BASELINE.json configs[2], the 28-qubit Fermi-Hubbard chain
+(sector dim 11,778,624; 188.5 MB per vector, larger than the 126 MB L2, so no L2 flush is needed).
+A "step" is one pass of the hot path over one state vector: one order-12 shifted Taylor step of
+exp(-i H dt) (a7: 12 fused apply+axpy launches of the a4 kernel) followed by one fused energy
+(a5: bs_expect) = 13 H applications.  a1-a3 (grouping, sector tables) are built once per operator and
+reported as setup_ms; a6 (rotations) is timed in the q24 entry of `per_config`.
+value = H applications per second over all ranks (each rank propagates its own state: weak scaling,
+no data-path collective).  See DESIGN.md "Measurement" for the byte counts behind `roofline`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import synth_inputs as si  # noqa: E402
+
+METRIC = "H|psi> applies/s (fp64 complex)"
+UNIT = "applies/s"
+TAYLOR_ORDER = 12
+DT = 0.05
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])), mx.append(float(f[1])), pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_operator_terms(name: str):
+    """Raw JW term lists of a config (host, numpy) -- the input of bs_group_xmask."""
+    from paper_2606_28952_b200 import jw_terms as jw
+    cfg = si.CONFIGS[name]
+    if cfg.kind == "hubbard":
+        return jw.hubbard_raw_terms(cfg.n_orb, cfg.hubbard_t, cfg.hubbard_u)
+    h, g = si.integrals(cfg.n_orb, cfg.seed_ints)
+    return jw.molecular_raw_terms(h, g)
+
+
+def table_bytes(op) -> int:
+    """Group-table bytes of the a2 layout: xg u64[G] + offs i64[G+1] + z u64[M] + w c128[M]."""
+    return 8 * op.n_groups + 8 * (op.n_groups + 1) + 24 * op.n_terms
+
+
+def _median(v):
+    return float(np.median(np.asarray(v, dtype=np.float64)))
+
+
+def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
+    """Plain bs_apply / bs_expect timings of one BASELINE.json config (CUDA events, median)."""
+    cfg = si.CONFIGS[name]
+    t0 = time.perf_counter()
+    raw = build_operator_terms(name)
+    t_raw = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    op = bs.bs_group_xmask(*raw, cfg.n_qubits, 1e-12)
+    sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t0
+    m_raw = len(raw[0])
+    del raw
+    psi = torch.from_numpy(si.random_state(cfg.dim, cfg.seed_psi)).cuda()
+    out = torch.empty_like(psi)
+    flush = 16 * cfg.dim * 2 < 126e6                      # both vectors would sit in the 126 MB L2
+    ev = lambda: torch.cuda.Event(enable_timing=True)     # noqa: E731
+    a, b = ev(), ev()
+    a.record()
+    bs.bs_apply(op, sec, psi, out)                         # first call also builds the cached plan
+    b.record()
+    torch.cuda.synchronize()
+    first_ms = a.elapsed_time(b)
+    reps = 0 if first_ms > 20000 else (3 if first_ms > 500 else 10)
+    times = []
+    for _ in range(reps):
+        if flush:
+            flush_buf.zero_()
+        a, b = ev(), ev()
+        a.record()
+        bs.bs_apply(op, sec, psi, out)
+        b.record()
+        torch.cuda.synchronize()
+        times.append(a.elapsed_time(b))
+    apply_ms = _median(times) if times else first_ms
+    ent = {"n_qubits": cfg.n_qubits, "dim": cfg.dim, "groups": op.n_groups, "strings": op.n_terms,
+           "raw_terms": m_raw, "raw_terms_s": round(t_raw, 3), "setup_s": round(t_setup, 3),
+           "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
+           "l2_flush_between_reps": bool(flush)}
+    bytes_alg = 32 * cfg.dim + table_bytes(op)
+    ent["hbm_gbs_algorithmic"] = bytes_alg / apply_ms / 1e6
+    ent["hbm_frac_of_measured_peak"] = ent["hbm_gbs_algorithmic"] / peak_gbs
+    if reps:
+        t0 = time.perf_counter()
+        e = bs.bs_expect(op, sec, psi)
+        ent["expect_ms"] = (time.perf_counter() - t0) * 1e3
+        ent["energy"] = e.real
+    if name == "q24":
+        from paper_2606_28952_b200 import jw_terms as jw
+        ex = si.uccsd_excitations(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+        th = si.thetas(len(ex), cfg.seed_theta)
+        X, Z, Cc, offs = jw.excitation_generator_terms(ex)
+        gens = bs.bs_group_xmask(X, Z, Cc, cfg.n_qubits, 0.0, bs.BS_MODE_SEQUENCE, offs)
+        rt = []
+        for i in range(4):
+            psi.zero_()
+            psi[0] = 1.0
+            a, b = ev(), ev()
+            a.record()
+            bs.bs_apply_pauli_rotations(gens, sec, th, psi)
+            b.record()
+            torch.cuda.synchronize()
+            if i:
+                rt.append(a.elapsed_time(b))
+        ent["uccsd_prep_ms"] = _median(rt)
+        ent["rotations_per_s"] = len(ex) / (_median(rt) * 1e-3)
+    del psi, out, op, sec
+    torch.cuda.empty_cache()
+    return ent
+
+
+def cpu_baseline(name: str, max_seconds: float = 30.0):
+    """The oracle's grouped apply (OpenMP over targets, as it stands) on this host's cores.
+    One apply of the workload when that fits the budget, else an alpha-row slab scaled linearly in rows."""
+    from oracle import oracle as orc
+    cfg = si.CONFIGS[name]
+    if cfg.kind == "hubbard":
+        ref = orc.hubbard_h(cfg.n_orb, cfg.hubbard_t, cfg.hubbard_u)
+    else:
+        ref = orc.molecular_h(*si.integrals(cfg.n_orb, cfg.seed_ints))
+    osec = orc.Sector(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    psi = si.random_state(cfg.dim, cfg.seed_psi)
+    out = np.zeros_like(psi)
+    rows = osec.dim_alpha
+    probe = max(1, rows // 64)
+    t0 = time.perf_counter()
+    osec.apply_grouped(ref, psi, 0, probe, out)
+    t_probe = time.perf_counter() - t0
+    n_rows = int(min(rows, max(probe, (max_seconds * 0.6) / (t_probe / probe))))
+    t0 = time.perf_counter()
+    osec.apply_grouped(ref, psi, 0, n_rows, out)
+    t = time.perf_counter() - t0
+    applies_per_s = (n_rows / rows) / t
+    sample = (f"oracle orc_apply_grouped on alpha rows [0,{n_rows}) of {rows} ({n_rows * osec.dim_beta} of "
+              f"{cfg.dim} targets) in {t:.2f} s, scaled linearly in rows")
+    return {"value": applies_per_s, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_28952_b200 import bs          # raises if libbs.so is missing: no CPU fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (libbs has no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peak_gbs, peak_src = _peaks()
+    name = args.workload
+    cfg = si.CONFIGS[name]
+    D = cfg.dim
+
+    # ---- setup (a1-a3), outside the timed region ------------------------------------------------
+    t0 = time.perf_counter()
+    raw = build_operator_terms(name)
+    op = bs.bs_group_xmask(*raw, cfg.n_qubits, 1e-12)
+    sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    torch.cuda.synchronize()
+    setup_ms = (time.perf_counter() - t0) * 1e3
+    del raw
+    psi_h = torch.from_numpy(si.random_state(D, cfg.seed_psi + rank)).pin_memory()   # one state per rank
+    out_h = torch.empty_like(psi_h).pin_memory()
+    psi = psi_h.cuda()
+    work = torch.empty(2 * D, dtype=torch.complex128, device="cuda")
+    e_shift = bs.bs_expect(op, sec, psi).real            # also builds the cached plan
+    tb = table_bytes(op)
+    ev = lambda: torch.cuda.Event(enable_timing=True)    # noqa: E731
+
+    def step():
+        bs.bs_taylor_step(op, sec, psi, work, DT, TAYLOR_ORDER, e_shift)
+        return bs.bs_expect(op, sec, psi)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ------------------------------------------------------------------
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    n0 = bs.bs_launch_count()
+    marks = [ev() for _ in range(2 * args.steps + 1)]
+    marks[0].record()
+    energy = None
+    for i in range(args.steps):
+        bs.bs_taylor_step(op, sec, psi, work, DT, TAYLOR_ORDER, e_shift)
+        marks[2 * i + 1].record()
+        energy = bs.bs_expect(op, sec, psi)
+        marks[2 * i + 2].record()
+    barrier()
+    launches = bs.bs_launch_count() - n0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = marks[0].elapsed_time(marks[-1])
+    taylor_ms = sum(marks[2 * i].elapsed_time(marks[2 * i + 1]) for i in range(args.steps))
+    expect_ms = sum(marks[2 * i + 1].elapsed_time(marks[2 * i + 2]) for i in range(args.steps))
+    norm_drift = abs(bs.bs_vdot(sec, psi, psi).real - 1.0)
+
+    # ---- end to end: host buffers, H2D + D2H inside the timed region ---------------------------------
+    e2e_steps = max(1, min(args.steps, 10))
+    psi.copy_(psi_h)
+    barrier()
+    a, b = ev(), ev()
+    a.record()
+    for _ in range(e2e_steps):
+        psi.copy_(psi_h, non_blocking=True)
+        step()
+        out_h.copy_(psi, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+    b.record()
+    barrier()
+    e2e_ms = a.elapsed_time(b)
+
+    t = torch.tensor([total_ms, e2e_ms, taylor_ms, expect_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms, taylor_ms, expect_ms = t.tolist()
+    applies_per_step = TAYLOR_ORDER + 1
+    if rank == 0:
+        value = world * applies_per_step * args.steps / (total_ms * 1e-3)
+        # dominant kernel: k_apply_sector (Taylor launches). Algorithmic bytes per Taylor step:
+        # k=1: 32 D; k=2..order-1: 64 D (in, out, acc r+w); k=order: 48 D; + tables each launch.
+        bytes_taylor = (32 + 64 * (TAYLOR_ORDER - 2) + 48) * D + TAYLOR_ORDER * tb
+        launch_ms = taylor_ms / (args.steps * TAYLOR_ORDER)
+        achieved = bytes_taylor / TAYLOR_ORDER / launch_ms / 1e6
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": f"{name}: BASELINE.json configs[{si.CONFIG_ORDER.index(name)}]",
+                       "n_qubits": cfg.n_qubits, "sector": [cfg.n_orb, cfg.n_alpha, cfg.n_beta], "dim": D,
+                       "groups": op.n_groups, "strings": op.n_terms,
+                       "step": f"1 Taylor-{TAYLOR_ORDER} step (dt={DT}, shifted) + 1 bs_expect = "
+                               f"{applies_per_step} H applies",
+                       "l2": "3 vectors x 188.5 MB > 126 MB L2, no flush needed",
+                       "parallelism": f"{world} independent state vector(s), one per GPU"},
+            "setup_ms": setup_ms, "taylor_ms_per_step": taylor_ms / args.steps,
+            "expect_ms_per_call": expect_ms / args.steps, "energy": energy.real, "norm_drift": norm_drift,
+            "gpu_launches": int(launches), "clocks": clocks,
+            "e2e": {"value": world * applies_per_step * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": 16 * D, "d2h_bytes_per_step": 16 * D + 16, "steps": e2e_steps},
+            "roofline": {"bound": "hbm", "kernel": "k_apply_sector (fused apply+axpy launches of bs_taylor_step)",
+                         "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
+                         "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
+                         "launch_ms": launch_ms, "traffic": TRAFFIC_NCU.get(name)},
+        }
+        want = [] if args.per_config == "none" else args.per_config.split(",")
+        if want and world == 1:
+            del psi, work
+            torch.cuda.empty_cache()
+            flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+            line["per_config"] = {n: per_config_entry(n, bs, torch, peak_gbs, flush_buf) for n in want}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(name)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until a capture exists for that workload.
+TRAFFIC_NCU = {}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands (OpenMP grouped apply) on this host's cores.
+    Each step is one H application on a bounded sample (an alpha-row slab) of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    name = args.workload
+    cfg = si.CONFIGS[name]
+    if cfg.kind == "hubbard":
+        ref = orc.hubbard_h(cfg.n_orb, cfg.hubbard_t, cfg.hubbard_u)
+    else:
+        ref = orc.molecular_h(*si.integrals(cfg.n_orb, cfg.seed_ints))
+    osec = orc.Sector(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    psi = si.random_state(cfg.dim, cfg.seed_psi)
+    out = np.zeros_like(psi)
+    rows = osec.dim_alpha
+    probe = max(1, rows // 64)
+    t0 = time.perf_counter()
+    osec.apply_grouped(ref, psi, 0, probe, out)
+    per_row = (time.perf_counter() - t0) / probe
+    budget = 150.0 / max(1, args.steps + args.warmup)      # whole run within a few minutes
+    n_rows = int(min(rows, max(1, budget / per_row)))
+    for _ in range(args.warmup):
+        osec.apply_grouped(ref, psi, 0, n_rows, out)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        osec.apply_grouped(ref, psi, 0, n_rows, out)
+    t = time.perf_counter() - t0
+    value = args.steps * (n_rows / rows) / t
+    sample = f"alpha rows [0,{n_rows}) of {rows} per step, scaled linearly in rows"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": f"{name}: BASELINE.json configs[{si.CONFIG_ORDER.index(name)}]",
+                       "n_qubits": cfg.n_qubits, "sector": [cfg.n_orb, cfg.n_alpha, cfg.n_beta], "dim": cfg.dim,
+                       "step": "1 H application by the CPU oracle (orc_apply_grouped) on a row slab"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "kind": "oracle", "cores": orc.num_threads(),
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="q28_hubbard", choices=si.CONFIG_ORDER)
+    ap.add_argument("--per-config", default="q12,q24,q28_hubbard,q32",
+                    help="comma list of configs to time with plain bs_apply (N=1 only), or 'none'")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
