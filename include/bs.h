@@ -121,6 +121,10 @@ int bs_apply_pauli_rotations(bs_op_t generators, bs_sector_t s, const double* th
 int bs_taylor_step(bs_op_t op, bs_sector_t s, void* psi_inout, void* work, double dt, int order,
                    double e_shift, void* cuda_stream);
 
+/* Human-readable description of the cached (op, sector) plan (kernel path, table sizes, launch
+ * geometry) written to buf [host] (at most n bytes, NUL terminated); builds the plan if needed. */
+int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n, void* cuda_stream);
+
 /* number of kernels this library has launched in this process (for bench.py's gpu_launches) */
 int64_t bs_launch_count(void);
 const char* bs_last_error(void);

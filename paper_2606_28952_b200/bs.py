@@ -25,7 +25,7 @@ SYMBOLS = [
     "bs_group_xmask", "bs_op_info", "bs_op_export", "bs_op_destroy",
     "bs_sector_build", "bs_sector_info", "bs_sector_export", "bs_sector_rank", "bs_sector_destroy",
     "bs_apply", "bs_apply_rows", "bs_apply_axpby", "bs_expect", "bs_vdot",
-    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_launch_count", "bs_last_error", "bs_version",
+    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_launch_count", "bs_last_error", "bs_version",
 ]
 
 
@@ -58,6 +58,7 @@ def _load():
     L.bs_vdot.argtypes = [vp, vp, vp, C.POINTER(dbl), vp]
     L.bs_apply_pauli_rotations.argtypes = [vp, vp, vp, i64, vp, vp]
     L.bs_taylor_step.argtypes = [vp, vp, vp, vp, dbl, C.c_int, dbl, vp]
+    L.bs_plan_describe.argtypes = [vp, vp, C.c_char_p, i64, vp]
     L.bs_launch_count.restype = i64
     L.bs_last_error.restype = C.c_char_p
     L.bs_version.restype = C.c_char_p
@@ -243,3 +244,9 @@ def bs_taylor_step(op: Op, sector: Sector, psi, work, dt: float, order: int = 12
     _check(_lib.bs_taylor_step(op._h, sector._h, _dev_ptr(psi, sector.dim, "psi"),
                                _dev_ptr(work, 2 * sector.dim, "work"), dt, order, e_shift, _stream(stream)))
     return psi
+
+
+def bs_plan_describe(op: Op, sector: Sector, stream=None) -> str:
+    buf = C.create_string_buffer(1024)
+    _check(_lib.bs_plan_describe(op._h, sector._h, buf, 1024, _stream(stream)))
+    return buf.value.decode()

@@ -13,81 +13,18 @@
 // load and accumulates in registers.  Groups with x_b = 0 read their source row contiguously.
 #include <algorithm>
 
+#include "bs_epilogue.cuh"
 #include "bs_plan.cuh"
 
 extern const int kFullChunkStrings;
+int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i64 lo, i64 hi, const Epilogue& ep,
+                  bool expect, cudaStream_t st, i64* n_partials_out, double2** partials_out);
 
 namespace {
 
 constexpr int kThreads = 256;
 constexpr int kCpt = 2;  // columns per thread
 constexpr int kColsPerBlock = kThreads * kCpt;
-
-struct Epilogue {
-    double2 alpha, beta, scale;  // out = scale * (alpha * Hpsi + beta * psi_in [+ acc stuff])
-    double2* acc;                // optional accumulator: acc += out (+ psi_in if add_in)
-    int use_axpby;               // 0: out = Hpsi
-    int add_in;                  // acc += out + psi_in
-    int store_out;               // write out
-    int scale_acc;               // acc = scale * (acc + out ...) instead of scaling out
-};
-
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-__device__ __forceinline__ double flip(double v, u32 par) {  // (-1)^par * v by a sign-bit XOR
-    return __hiloint2double(__double2hiint(v) ^ (int)(par << 31), __double2loint(v));
-}
-
-// block-wide deterministic sum of one double2 per thread -> thread 0
-__device__ __forceinline__ double2 block_sum(double2 v, double2* sh) {
-    for (int o = 16; o > 0; o >>= 1) {
-        v.x += __shfl_down_sync(0xffffffffu, v.x, o);
-        v.y += __shfl_down_sync(0xffffffffu, v.y, o);
-    }
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    if (l == 0) sh[w] = v;
-    __syncthreads();
-    if (w == 0) {
-        int nw = (blockDim.x + 31) >> 5;
-        v = (l < nw) ? sh[l] : make_double2(0.0, 0.0);
-        for (int o = 16; o > 0; o >>= 1) {
-            v.x += __shfl_down_sync(0xffffffffu, v.x, o);
-            v.y += __shfl_down_sync(0xffffffffu, v.y, o);
-        }
-    }
-    return v;
-}
-
-template <bool EXPECT>
-__device__ __forceinline__ void finish_target(double2 a, double2 pin, i64 idx, double2* __restrict__ out,
-                                              const Epilogue& ep, double2& dot) {
-    if (EXPECT) {
-        // conj(psi) * Hpsi
-        dot.x += pin.x * a.x + pin.y * a.y;
-        dot.y += pin.x * a.y - pin.y * a.x;
-        return;
-    }
-    if (ep.use_axpby) {
-        double2 r = cmul(ep.alpha, a), b = cmul(ep.beta, pin);
-        r.x += b.x;
-        r.y += b.y;
-        if (ep.acc) {
-            double2 c = ep.acc[idx];
-            c.x += r.x;
-            c.y += r.y;
-            if (ep.add_in) {
-                c.x += pin.x;
-                c.y += pin.y;
-            }
-            if (ep.scale_acc) c = cmul(ep.scale, c);
-            ep.acc[idx] = c;
-        }
-        if (ep.store_out) out[idx] = r;
-    } else {
-        out[idx] = a;
-    }
-}
 
 template <bool EXPECT, bool REALW>
 __global__ void __launch_bounds__(kThreads)
@@ -154,33 +91,6 @@ k_apply_sector(SpinTab A, SpinTab B, const u32* __restrict__ ga_off, const uint4
         if (threadIdx.x == 0) partials[(i64)blockIdx.y * gridDim.x + blockIdx.x] = dot;
     }
 }
-
-// ---- TMA bulk-copy + mbarrier helpers (cp.async.bulk, SASS: UBLKCP) -----------------------------
-__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, u32 bytes, u64* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ u32 round16(u32 b) { return (b + 15u) & ~15u; }
 
 // Full-space kernel (n_alpha = n_beta = -1): index = configuration word, every group is valid for
 // every target.  One thread per target; the group/string tables are streamed through shared
@@ -317,6 +227,7 @@ int launch_apply(bs_op* op, bs_sector* s, const double2* psi, double2* out, i64 
         if (n_partials_out) *n_partials_out = 0;
         return BS_OK;
     }
+    if (!s->full && P->rp_main) return bs_rows_apply(P, s, psi, out, lo, hi, ep, expect, st, n_partials_out, partials_out);
     if (s->full) {
         BS_REQUIRE(kFullChunkStrings == kFullStr, BS_ERR_ARG, "internal: chunk size mismatch");
         i64 nblk = (hi - lo + kThreads - 1) / kThreads;

@@ -6,6 +6,7 @@
 #include <algorithm>
 
 #include "bs_plan.cuh"
+#include "bs_rowplan.cuh"
 
 namespace {
 
@@ -39,14 +40,45 @@ __global__ void k_row_fill(SpinTab A, const u32* __restrict__ xa, int n_xa, cons
     }
 }
 
-struct HostStr {
-    u32 za, zb;
-    double re, im;
-};
-struct HostGroup {
-    u32 xa, xb;
-    std::vector<HostStr> s;
-};
+// v2 row plans.  B groups (xa = 0, xb != 0) stay in the main plan (same-row gathers from the staged
+// row) when they are few; when they are many (molecular Hamiltonians: all beta single and double
+// excitations) they are applied as A groups of the transposed problem, where the gather becomes a
+// coalesced row read.  Any failure (tables too large, ...) leaves the v1 kernel in charge.
+void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st) {
+    const char* force = getenv("BS_KERNEL");
+    if (force && std::string(force) == "v1") return;
+    if (S->Da > 32767 || S->Db > 32767) return;
+    size_t nB = 0;
+    for (auto& g : groups) nB += (g.xa == 0 && g.xb != 0);
+    const bool transposed_b = nB > 64 && !(force && std::string(force) == "v2inrow");
+    std::vector<HostGroup> main_g, t_g;
+    for (auto& g : groups) {
+        if (transposed_b && g.xa == 0 && g.xb != 0) {
+            HostGroup t;
+            t.xa = g.xb;
+            t.xb = 0;
+            for (auto& s : g.s) t.s.push_back(HostStr{s.zb, s.za, s.re, s.im});
+            std::stable_sort(t.s.begin(), t.s.end(), [](const HostStr& a, const HostStr& b) {
+                return a.zb < b.zb || (a.zb == b.zb && a.za < b.za);
+            });
+            t_g.push_back(std::move(t));
+        } else main_g.push_back(g);
+    }
+    std::stable_sort(t_g.begin(), t_g.end(), [](const HostGroup& a, const HostGroup& b) { return a.xa < b.xa; });
+    bs_rowplan* m = new (std::nothrow) bs_rowplan;
+    bs_rowplan* t = t_g.empty() ? nullptr : new (std::nothrow) bs_rowplan;
+    bool ok = m && (t_g.empty() || t);
+    if (ok) ok = bs_rowplan_build(m, main_g, S->ta, S->tb, st) == BS_OK;
+    if (ok && t) ok = bs_rowplan_build(t, t_g, S->tb, S->ta, st) == BS_OK;
+    if (!ok) {
+        cudaGetLastError();
+        bs_rowplan_free(m);
+        bs_rowplan_free(t);
+        return;
+    }
+    P->rp_main = m;
+    P->rp_t = t;
+}
 
 int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
     const int n = S->n_orb;
@@ -93,6 +125,7 @@ int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
     std::stable_sort(groups.begin(), groups.end(), [](const HostGroup& a, const HostGroup& b) {
         return a.xa < b.xa || (a.xa == b.xa && a.xb < b.xb);
     });
+    build_row_plans(P, groups, S, st);
     std::vector<u32> xa_list, ga_off;
     std::vector<uint4> hdr;
     std::vector<uint2> szab;
@@ -201,6 +234,12 @@ int bs_plan_get(bs_op* op, bs_sector* s, cudaStream_t st, bs_plan** out) {
     return BS_OK;
 }
 
+bs_plan::~bs_plan() {
+    bs_rowplan_free(rp_main);
+    bs_rowplan_free(rp_t);
+}
+void bs_rowplan_free(bs_rowplan* R) { delete R; }
+
 void bs_plan_purge(u64 op_id, u64 sector_id) {
     std::lock_guard<std::mutex> lk(g_plan_mu);
     for (auto it = g_plans.begin(); it != g_plans.end();) {
@@ -209,4 +248,33 @@ void bs_plan_purge(u64 op_id, u64 sector_id) {
             it = g_plans.erase(it);
         } else ++it;
     }
+}
+
+extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n, void* cuda_stream) {
+    BS_REQUIRE(op && s && buf && n > 0, BS_ERR_ARG, "bs_plan_describe: bad argument");
+    bs_plan* P = nullptr;
+    int rc = bs_plan_get(op, s, (cudaStream_t)cuda_stream, &P);
+    if (rc != BS_OK) return rc;
+    if (P->full) {
+        snprintf(buf, (size_t)n, "kernel=full chunks=%d real_w=%d", P->n_chunks, (int)P->real_w);
+    } else if (P->rp_main) {
+        const bs_rowplan* M = P->rp_main;
+        const bs_rowplan* T = P->rp_t;
+        int w = snprintf(buf, (size_t)n,
+                         "kernel=rows_v2 real_w=%d main{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d "
+                         "row_ent=%lld threads=%d cpt=%d chunk_cols=%d win_cols=%d n_win=%d smem=%zu}",
+                         (int)M->real_w, M->n_xa, (long long)M->n_items, (long long)M->n_keys, (long long)M->n_strings,
+                         (long long)M->n_tkeys, M->max_keys, (long long)M->n_row_ent, M->threads, M->cpt, M->chunk_cols,
+                         M->win_cols, M->n_win, M->smem);
+        if (T && w > 0 && w < n)
+            snprintf(buf + w, (size_t)(n - w),
+                     " transposed{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d row_ent=%lld threads=%d "
+                     "cpt=%d chunk_cols=%d smem=%zu}",
+                     T->n_xa, (long long)T->n_items, (long long)T->n_keys, (long long)T->n_strings, (long long)T->n_tkeys,
+                     T->max_keys, (long long)T->n_row_ent, T->threads, T->cpt, T->chunk_cols, T->smem);
+    } else {
+        snprintf(buf, (size_t)n, "kernel=sector_v1 real_w=%d xa=%d groups=%lld strings=%lld row_ent=%lld", (int)P->real_w,
+                 P->n_xa, (long long)P->n_groups, (long long)P->n_strings, (long long)P->n_row_ent);
+    }
+    return BS_OK;
 }

@@ -9,7 +9,23 @@ struct FullChunk {
     int s0, s1;  // string range
 };
 
+// host-side group after z-reduction (bs_plan.cu), oriented: xa acts on the row spin, xb on the column spin
+struct HostStr {
+    u32 za, zb;
+    double re, im;
+};
+struct HostGroup {
+    u32 xa, xb;
+    std::vector<HostStr> s;  // sorted by (zb, za), merged, non-zero
+};
+
+struct bs_rowplan;
+int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const SpinTab& A, const SpinTab& B,
+                     cudaStream_t st);
+void bs_rowplan_free(bs_rowplan* R);
+
 struct bs_plan {
+    ~bs_plan();
     u64 op_id = 0, sector_id = 0;
     bool full = false;
     bool real_w = false;  // every weight has zero imaginary part (Hermitian real-coefficient H)
@@ -34,6 +50,11 @@ struct bs_plan {
     std::vector<FullChunk> h_chunks;
     DevBuf<FullChunk> d_chunks;
     int n_chunks = 0;
+
+    // ---- v2 row plans (bs_rowplan.cuh); null -> the v1 kernel is used --------------------------------
+    bs_rowplan* rp_main = nullptr;  // D, A, AB groups (and B groups when they are few)
+    bs_rowplan* rp_t = nullptr;     // B groups as A groups of the transposed problem (when they are many)
+    DevBuf<double2> d_psi_t, d_out_t, d_raw;  // transposed input / output, raw H psi (lazily allocated)
 
     // partial sums of bs_expect, one per thread block of the apply grid
     DevBuf<double2> d_partials;

@@ -1,0 +1,341 @@
+// a4 apply, v2 row kernel (Eq. 27; Eq. 28).
+//
+// One thread block owns one target row t_a and a chunk of target columns t_b; every thread owns up
+// to CPT columns and keeps their accumulators in registers.  For every alpha mask x_a that is valid
+// for the row (precomputed list: mask id, source row) the block
+//   1. evaluates the row-dependent phase factors V_gj(t_a) of all groups under x_a into shared
+//      memory (one per KEY = distinct beta Z mask of a group; strings are visited once per row, not
+//      once per target),
+//   2. if some group under x_a moves the beta string, stages the source row psi[u_a, :] in shared
+//      memory with TMA bulk copies (cp.async.bulk + mbarrier), in windows if the row is larger than
+//      shared memory,
+//   3. walks the groups: one coalesced u16 load from the column table gives validity, source column
+//      and the first sign; remaining keys cost one AND + bit test (or POPC) + sign flip + add; the
+//      source amplitude is a 128-bit shared-memory gather (x_b != 0) or a coalesced 128-bit global
+//      load (x_b = 0: same column of another row), then two (real V) or four FMAs.
+// No tensor cores: this is a gather with integer bit math (north star).
+#include <algorithm>
+
+#include "bs_epilogue.cuh"
+#include "bs_plan.cuh"
+#include "bs_rowplan.cuh"
+
+namespace {
+
+constexpr int MODE_FINAL = 0, MODE_RAW = 1, MODE_EXPECT = 2;
+
+template <bool REALW>
+struct VT;
+template <>
+struct VT<true> {
+    using type = double;
+    static __device__ __forceinline__ double zero() { return 0.0; }
+    static __device__ __forceinline__ void addflip(double& f, double v, u32 par) { f += flip(v, par); }
+    static __device__ __forceinline__ void fma(double2& acc, double f, u32 sg, double2 a) {
+        f = flip(f, sg);
+        acc.x += f * a.x;
+        acc.y += f * a.y;
+    }
+    static __device__ __forceinline__ double from(double2 w) { return w.x; }
+};
+template <>
+struct VT<false> {
+    using type = double2;
+    static __device__ __forceinline__ double2 zero() { return make_double2(0.0, 0.0); }
+    static __device__ __forceinline__ void addflip(double2& f, double2 v, u32 par) {
+        f.x += flip(v.x, par);
+        f.y += flip(v.y, par);
+    }
+    static __device__ __forceinline__ void fma(double2& acc, double2 f, u32 sg, double2 a) {
+        f.x = flip(f.x, sg);
+        f.y = flip(f.y, sg);
+        acc.x += f.x * a.x - f.y * a.y;
+        acc.y += f.x * a.y + f.y * a.x;
+    }
+    static __device__ __forceinline__ double2 from(double2 w) { return w; }
+};
+
+// CPT packed u16 table entries of one thread (the table is stored thread-blocked, see bs_rowplan.cu)
+template <int CPT>
+__device__ __forceinline__ void load_entries(const unsigned short* __restrict__ p, u32 (&e)[CPT]) {
+    if (CPT == 4) {
+        const uint2 v = __ldg(reinterpret_cast<const uint2*>(p));
+        e[0] = v.x & 0xFFFFu;
+        e[1] = v.x >> 16;
+        e[2 % CPT] = v.y & 0xFFFFu;
+        e[3 % CPT] = v.y >> 16;
+    } else if (CPT == 2) {
+        const u32 v = __ldg(reinterpret_cast<const u32*>(p));
+        e[0] = v & 0xFFFFu;
+        e[1 % CPT] = v >> 16;
+    } else {
+        e[0] = __ldg(p);
+    }
+}
+
+// sum over the remaining keys of a multi-key group: f += sum_j (+-) V_j, sign from the column string
+template <bool REALW>
+__device__ __forceinline__ typename VT<REALW>::type multi_key(typename VT<REALW>::type f,
+                                                              const typename VT<REALW>::type* __restrict__ v,
+                                                              const u32* __restrict__ dz, u32 nkeys, u32 single, u32 tb) {
+    using V = VT<REALW>;
+    if (single) {
+        for (u32 j = 1; j < nkeys; ++j) V::addflip(f, v[j], (tb & __ldg(dz + j)) ? 1u : 0u);
+    } else {
+        for (u32 j = 1; j < nkeys; ++j) V::addflip(f, v[j], (u32)__popc(tb & __ldg(dz + j)) & 1u);
+    }
+    return f;
+}
+
+template <int MODE, bool REALW, int CPT, int MAXT>
+__global__ void __launch_bounds__(MAXT)
+k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict__ out, i64 row_lo, i64 col_lo,
+       i64 col_hi, int chunk0, Epilogue ep, double2* __restrict__ partials) {
+    using V = VT<REALW>;
+    using vt = typename V::type;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ double2 sh_red[32];
+    u64* bar = reinterpret_cast<u64*>(smem_raw);
+    vt* sV = reinterpret_cast<vt*>(smem_raw + 16);
+    double2* srow = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)P.max_keys * 16);
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const i64 row = row_lo + blockIdx.x;
+    const u32 Db = (u32)P.B.D;
+    const u32 ta = P.A.str[row];
+    const u32 chunk = (u32)chunk0 + blockIdx.y;
+    const u32 c0 = chunk * (u32)P.chunk_cols;
+    const u32 tpos = (chunk * (u32)nt + (u32)tid) * CPT;  // this thread's slot in a thread-blocked table row
+    u32 col[CPT], tb[CPT];
+    bool ok[CPT];
+    double2 acc[CPT];
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+        const u32 cc = c0 + (u32)tid + (u32)c * (u32)nt;
+        ok[c] = cc < c0 + (u32)P.chunk_cols && cc < Db && (i64)cc >= col_lo && (i64)cc < col_hi;
+        col[c] = min(cc, Db - 1u);  // clamped: loads stay in range, results of !ok columns are never stored
+        tb[c] = P.B.str[col[c]];
+        acc[c] = make_double2(0.0, 0.0);
+    }
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    u32 phase = 0;
+    const uint4* __restrict__ items4 = reinterpret_cast<const uint4*>(P.items);
+    const i64 e0 = P.row_off[row], e1 = P.row_off[row + 1];
+    for (i64 e = e0; e < e1; ++e) {
+        const uint2 ent = __ldg(P.row_ent + e);
+        const uint4 h4 = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + ent.x));      // item0,item1,key0,key1
+        const u32 stage = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + ent.x) + 4);
+        const u32 item0 = h4.x, item1 = h4.y, key0 = h4.z, key1 = h4.w;
+        const double2* __restrict__ srcp = psi + (i64)ent.y * Db;
+        const int n_win = stage ? P.n_win : 1;
+        __syncthreads();  // everyone is done with the previous entry's V slots and staged row
+        for (int w = 0; w < n_win; ++w) {
+            const u32 w0 = (u32)w * (u32)P.win_cols;
+            const u32 wn = stage ? min((u32)P.win_cols, Db - w0) : 0u;
+            if (stage) {
+                if (w > 0) __syncthreads();  // readers of the previous window are done
+                if (tid == 0) {
+                    const u32 bytes = wn * 16u;
+                    mbar_expect_tx(bar, bytes);
+                    for (u32 o = 0; o < bytes; o += 32768u)
+                        tma_bulk_g2s(reinterpret_cast<unsigned char*>(srow) + o,
+                                     reinterpret_cast<const unsigned char*>(srcp + w0) + o, min(32768u, bytes - o), bar);
+                }
+            }
+            if (w == 0) {
+                // phase factors of every key under this alpha mask (overlaps the bulk copy)
+                for (u32 k = key0 + tid; k < key1; k += nt) {
+                    vt f = V::zero();
+                    const u32 s1 = __ldg(P.key_s0 + k + 1);
+                    for (u32 s = __ldg(P.key_s0 + k); s < s1; ++s)
+                        V::addflip(f, V::from(__ldg(P.s_w + s)), (u32)__popc(__ldg(P.s_za + s) & ta) & 1u);
+                    sV[k - key0] = f;
+                }
+                __syncthreads();
+            }
+            if (stage) {
+                mbar_wait(bar, phase);
+                phase ^= 1u;
+            }
+            const bool windowed = stage && n_win > 1;
+            uint4 nxt = item0 < item1 ? __ldg(items4 + item0) : make_uint4(0, 0, 0, 0);
+            for (u32 i = item0; i < item1; ++i) {
+                const uint4 it = nxt;  // {tkey, key0, nkeys, single}
+                if (i + 1 < item1) nxt = __ldg(items4 + i + 1);
+                const vt* __restrict__ v = sV + (it.y - key0);
+                const vt f0 = v[0];
+                if (it.x == kTkeyIdent) {
+                    // x_b = 0, no beta sign on the first key: same column of the source row
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) {
+                        if (windowed && (col[c] - w0) >= wn) continue;
+                        vt f = f0;
+                        if (it.z > 1) f = multi_key<REALW>(f, v, P.key_dz + it.y, it.z, it.w, tb[c]);
+                        const double2 a = stage ? srow[col[c] - w0] : __ldg(srcp + col[c]);
+                        V::fma(acc[c], f, 0u, a);
+                    }
+                } else {
+                    u32 en[CPT];
+                    load_entries<CPT>(P.ttab + (i64)it.x * P.tstride + tpos, en);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) {
+                        const u32 src = en[c] & 0x7FFFu;
+                        if (en[c] == 0xFFFFu || (windowed && (src - w0) >= wn)) continue;
+                        vt f = f0;
+                        if (it.z > 1) f = multi_key<REALW>(f, v, P.key_dz + it.y, it.z, it.w, tb[c]);
+                        const double2 a = stage ? srow[src - w0] : __ldg(srcp + src);
+                        V::fma(acc[c], f, en[c] >> 15, a);
+                    }
+                }
+            }
+        }
+    }
+    double2 dot = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+        if (!ok[c]) continue;
+        const i64 idx = row * (i64)Db + col[c];
+        if (MODE == MODE_RAW) {
+            out[idx] = acc[c];
+        } else {
+            double2 pin = make_double2(0.0, 0.0);
+            if (MODE == MODE_EXPECT || ep.use_axpby) pin = psi[idx];
+            finish_target<MODE == MODE_EXPECT>(acc[c], pin, idx, out, ep, dot);
+        }
+    }
+    if (MODE == MODE_EXPECT) {
+        dot = block_sum(dot, sh_red);
+        if (tid == 0) partials[(i64)blockIdx.y * gridDim.x + blockIdx.x] = dot;
+    }
+}
+
+// out_t[c][r] = in[r][c] for a [R x C] row-major matrix of complex128 (32 x 32 tiles through shared
+// memory, both sides coalesced)
+__global__ void __launch_bounds__(256) k_transpose(const double2* __restrict__ in, double2* __restrict__ out_t, i64 R,
+                                                   i64 C) {
+    __shared__ double2 tile[32][33];
+    const i64 r0 = (i64)blockIdx.y * 32, c0 = (i64)blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int j = ty; j < 32; j += 8)
+        if (r0 + j < R && c0 + tx < C) tile[j][tx] = in[(r0 + j) * C + c0 + tx];
+    __syncthreads();
+    for (int j = ty; j < 32; j += 8)
+        if (c0 + j < C && r0 + tx < R) out_t[(c0 + j) * R + r0 + tx] = tile[tx][j];
+}
+
+// Final pass when part of the operator ran on the transposed problem: for rows [row_lo, row_hi)
+//   H psi [r][c] = raw[r][c] + out_t[c][r], then the fused epilogue (store / axpby / dot partial).
+template <bool EXPECT>
+__global__ void __launch_bounds__(256)
+k_transpose_add_finish(const double2* raw, const double2* __restrict__ out_t,
+                       const double2* __restrict__ psi, double2* out, i64 Da, i64 Db, i64 row_lo,
+                       i64 row_hi, Epilogue ep, double2* __restrict__ partials) {
+    __shared__ double2 tile[32][33];
+    __shared__ double2 sh_red[32];
+    const i64 r0 = row_lo + (i64)blockIdx.y * 32, c0 = (i64)blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int j = ty; j < 32; j += 8)  // tile[j][tx] = out_t[c0 + j][r0 + tx]
+        if (c0 + j < Db && r0 + tx < row_hi) tile[j][tx] = out_t[(c0 + j) * Da + r0 + tx];
+    __syncthreads();
+    double2 dot = make_double2(0.0, 0.0);
+    for (int j = ty; j < 32; j += 8) {
+        const i64 r = r0 + j, c = c0 + tx;
+        if (r < row_hi && c < Db) {
+            const i64 idx = r * Db + c;
+            double2 a = raw[idx];
+            const double2 b = tile[tx][j];
+            a.x += b.x;
+            a.y += b.y;
+            double2 pin = make_double2(0.0, 0.0);
+            if (EXPECT || ep.use_axpby) pin = psi[idx];
+            finish_target<EXPECT>(a, pin, idx, out, ep, dot);
+        }
+    }
+    if (EXPECT) {
+        dot = block_sum(dot, sh_red);
+        if (threadIdx.x == 0) partials[(i64)blockIdx.y * gridDim.x + blockIdx.x] = dot;
+    }
+}
+
+template <int MODE, bool REALW, int CPT>
+cudaError_t launch_k_rows_t(const bs_rowplan* R, dim3 grid, cudaStream_t st, const double2* psi, double2* out,
+                            i64 row_lo, i64 col_lo, i64 col_hi, int chunk0, const Epilogue& ep, double2* partials) {
+    if (R->threads > 256) {
+        auto k = k_rows<MODE, REALW, CPT, 1024>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
+    } else {
+        auto k = k_rows<MODE, REALW, CPT, 256>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
+    }
+    return cudaGetLastError();
+}
+
+template <int MODE>
+cudaError_t launch_k_rows(const bs_rowplan* R, cudaStream_t st, const double2* psi, double2* out, i64 row_lo,
+                          i64 row_hi, i64 col_lo, i64 col_hi, const Epilogue& ep, double2* partials) {
+    const int chunk0 = (int)(col_lo / R->chunk_cols);
+    const unsigned n_chunks = (unsigned)((col_hi - 1) / R->chunk_cols - chunk0 + 1);
+    dim3 grid((unsigned)(row_hi - row_lo), n_chunks);
+    BS_COUNT_LAUNCH(1);
+#define BS_ROWS(RW, C) launch_k_rows_t<MODE, RW, C>(R, grid, st, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials)
+    if (R->real_w) return R->cpt == 1 ? BS_ROWS(true, 1) : (R->cpt == 2 ? BS_ROWS(true, 2) : BS_ROWS(true, 4));
+    return R->cpt == 1 ? BS_ROWS(false, 1) : (R->cpt == 2 ? BS_ROWS(false, 2) : BS_ROWS(false, 4));
+#undef BS_ROWS
+}
+
+}  // namespace
+
+// Runs the v2 path for rows [lo, hi).  expect: dot partials instead of stores.
+int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i64 lo, i64 hi, const Epilogue& ep,
+                  bool expect, cudaStream_t st, i64* n_partials_out, double2** partials_out) {
+    bs_rowplan* M = P->rp_main;
+    const i64 Da = s->Da, Db = s->Db;
+    if (!P->rp_t) {
+        const i64 nblk = (hi - lo) * ((Db + M->chunk_cols - 1) / M->chunk_cols);
+        if (expect && P->n_partials < nblk) {
+            BS_CUDA(P->d_partials.alloc(nblk));
+            P->n_partials = nblk;
+        }
+        if (expect) BS_CUDA(launch_k_rows<MODE_EXPECT>(M, st, psi, out, lo, hi, 0, Db, ep, P->d_partials.p));
+        else BS_CUDA(launch_k_rows<MODE_FINAL>(M, st, psi, out, lo, hi, 0, Db, ep, nullptr));
+        if (n_partials_out) *n_partials_out = nblk;
+        if (partials_out) *partials_out = P->d_partials.p;
+        return BS_OK;
+    }
+    // part of the operator (beta-only groups) runs on the transposed problem
+    if (!P->d_psi_t.p) BS_CUDA(P->d_psi_t.alloc(s->D));
+    if (!P->d_out_t.p) BS_CUDA(P->d_out_t.alloc(s->D));
+    double2* raw = out;
+    if (expect || !ep.store_out) {
+        if (!P->d_raw.p) BS_CUDA(P->d_raw.alloc(s->D));
+        raw = P->d_raw.p;
+    }
+    dim3 tg((unsigned)((Db + 31) / 32), (unsigned)((Da + 31) / 32));
+    k_transpose<<<tg, 256, 0, st>>>(psi, P->d_psi_t.p, Da, Db);
+    BS_COUNT_LAUNCH(1);
+    BS_CUDA(cudaGetLastError());
+    Epilogue none = ep;
+    BS_CUDA(launch_k_rows<MODE_RAW>(M, st, psi, raw, lo, hi, 0, Db, none, nullptr));
+    BS_CUDA(launch_k_rows<MODE_RAW>(P->rp_t, st, P->d_psi_t.p, P->d_out_t.p, 0, Db, lo, hi, none, nullptr));
+    dim3 fg((unsigned)((Db + 31) / 32), (unsigned)((hi - lo + 31) / 32));
+    const i64 nblk = (i64)fg.x * fg.y;
+    if (expect && P->n_partials < nblk) {
+        BS_CUDA(P->d_partials.alloc(nblk));
+        P->n_partials = nblk;
+    }
+    if (expect)
+        k_transpose_add_finish<true><<<fg, 256, 0, st>>>(raw, P->d_out_t.p, psi, out, Da, Db, lo, hi, ep, P->d_partials.p);
+    else
+        k_transpose_add_finish<false><<<fg, 256, 0, st>>>(raw, P->d_out_t.p, psi, out, Da, Db, lo, hi, ep, nullptr);
+    BS_COUNT_LAUNCH(1);
+    BS_CUDA(cudaGetLastError());
+    if (n_partials_out) *n_partials_out = nblk;
+    if (partials_out) *partials_out = P->d_partials.p;
+    return BS_OK;
+}

@@ -1,0 +1,222 @@
+// Builder of the v2 row plan (bs_rowplan.cuh): items / keys / strings tables, per-column u16 source
+// tables, per-row valid alpha-mask lists and the launch geometry.
+// PAPER.md:227-231 (Eq. 28, spin-split masks), PAPER.md:247 and 253-265 (phase factorisation).
+#include <algorithm>
+#include <map>
+
+#include "bs_plan.cuh"
+#include "bs_rowplan.cuh"
+
+namespace {
+
+// Thread-blocked column table: slot (chunk*threads + tid)*cpt + c of row `key` describes column
+// col = chunk*chunk_cols + tid + c*threads: rank_B(tb ^ xb) | parity(zb0 & tb) << 15, or 0xFFFF if the column is
+// outside the chunk / the row, or tb ^ xb leaves the sector.
+__global__ void k_fill_ttab(SpinTab B, const uint2* __restrict__ keys, i64 tstride, int threads, int cpt,
+                            int chunk_cols, unsigned short* __restrict__ T) {
+    const i64 slot = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (slot >= tstride) return;
+    const uint2 k = keys[blockIdx.y];  // {xb, zb0}
+    const i64 per_chunk = (i64)threads * cpt;
+    const i64 chunk = slot / per_chunk, r = slot - chunk * per_chunk;
+    const i64 tid = r / cpt, c = r - tid * cpt;
+    const i64 lc = tid + c * threads;
+    const i64 col = chunk * chunk_cols + lc;
+    unsigned short e = 0xFFFFu;
+    if (lc < chunk_cols && col < B.D) {
+        const u32 tb = B.str[col];
+        if (2 * __popc(tb & k.x) == __popc(k.x))
+            e = (unsigned short)(spin_rank(B, tb ^ k.x) | ((u32)(__popc(tb & k.y) & 1) << 15));
+    }
+    T[(i64)blockIdx.y * tstride + slot] = e;
+}
+
+__global__ void k_row_count2(SpinTab A, const u32* __restrict__ xa, int n_xa, int* __restrict__ cnt) {
+    i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (r >= A.D) return;
+    u32 ta = A.str[r];
+    int c = 0;
+    for (int i = 0; i < n_xa; ++i) {
+        u32 m = __ldg(xa + i);
+        c += (2 * __popc(ta & m) == __popc(m));
+    }
+    cnt[r] = c;
+}
+
+__global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, int n_xa, const i64* __restrict__ off,
+                            uint2* __restrict__ ent) {
+    i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (r >= A.D) return;
+    u32 ta = A.str[r];
+    i64 o = off[r];
+    for (int i = 0; i < n_xa; ++i) {
+        u32 m = __ldg(xa + i);
+        if (2 * __popc(ta & m) == __popc(m)) ent[o++] = make_uint2((u32)i, spin_rank(A, ta ^ m));
+    }
+}
+
+}  // namespace
+
+// groups: already z-reduced, oriented (xa = row-spin mask, xb = column-spin mask), sorted by (xa, xb).
+int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const SpinTab& A, const SpinTab& B,
+                     cudaStream_t st) {
+    const i64 Da = A.D, Db = B.D;
+    BS_REQUIRE(Db <= 32767, BS_ERR_ARG, "row plan: column space too large for u16 tables");
+    std::vector<u32> xa_list, key_dz, key_s0, s_za;
+    std::vector<XaHdr> hdrs;
+    std::vector<RowItem> items;
+    std::vector<double2> s_w;
+    std::vector<uint2> tkeys;
+    std::map<std::pair<u32, u32>, u32> tkey_id;
+    bool real_w = true;
+    int max_keys = 0;
+    for (size_t g = 0; g < groups.size(); ++g) {
+        const HostGroup& hg = groups[g];
+        if (g == 0 || hg.xa != groups[g - 1].xa) {
+            if (!hdrs.empty()) {
+                hdrs.back().item1 = (u32)items.size();
+                hdrs.back().key1 = (u32)key_dz.size();
+            }
+            XaHdr h{};
+            h.item0 = (u32)items.size();
+            h.key0 = (u32)key_dz.size();
+            h.stage = 0;
+            hdrs.push_back(h);
+            xa_list.push_back(hg.xa);
+        }
+        // strings arrive sorted by (zb, za): bucket by zb
+        RowItem it{};
+        it.key0 = (u32)key_dz.size();
+        it.single = 1;
+        const u32 zb0 = hg.s.front().zb;
+        for (size_t k = 0; k < hg.s.size(); ++k) {
+            if (k == 0 || hg.s[k].zb != hg.s[k - 1].zb) {
+                const u32 dz = hg.s[k].zb ^ zb0;
+                key_dz.push_back(dz);
+                key_s0.push_back((u32)s_za.size());
+                if (k && __builtin_popcount(dz) != 1) it.single = 0;
+            }
+            s_za.push_back(hg.s[k].za);
+            s_w.push_back(make_double2(hg.s[k].re, hg.s[k].im));
+            if (hg.s[k].im != 0.0) real_w = false;
+        }
+        it.nkeys = (u32)key_dz.size() - it.key0;
+        if (hg.xb == 0 && zb0 == 0) it.tkey = kTkeyIdent;
+        else {
+            auto key = std::make_pair(hg.xb, zb0);
+            auto f = tkey_id.find(key);
+            if (f == tkey_id.end()) {
+                f = tkey_id.emplace(key, (u32)tkeys.size()).first;
+                tkeys.push_back(make_uint2(hg.xb, zb0));
+            }
+            it.tkey = f->second;
+        }
+        if (hg.xb != 0) hdrs.back().stage = 1;
+        items.push_back(it);
+    }
+    if (!hdrs.empty()) {
+        hdrs.back().item1 = (u32)items.size();
+        hdrs.back().key1 = (u32)key_dz.size();
+    }
+    key_s0.push_back((u32)s_za.size());
+    bool any_stage = false;
+    for (auto& h : hdrs) {
+        max_keys = std::max(max_keys, (int)(h.key1 - h.key0));
+        any_stage |= h.stage != 0;
+    }
+    R->real_w = real_w;
+    R->n_xa = (int)xa_list.size();
+    R->n_items = (i64)items.size();
+    R->n_keys = (i64)key_dz.size();
+    R->n_strings = (i64)s_za.size();
+    R->n_tkeys = (i64)tkeys.size();
+    R->max_keys = max_keys;
+    R->any_stage = any_stage;
+    // ---- launch geometry ---------------------------------------------------------------------
+    // Shared memory: [mbarrier 16 B][V slots: max_keys * 16 B][row window: win_cols * 16 B].
+    const size_t fixed = 16 + (size_t)std::max(max_keys, 1) * 16;
+    const size_t smem_max = 227 * 1024 - 1024;
+    i64 win = Db;
+    int n_win = 1;
+    if (any_stage) {
+        const i64 cap = (i64)((smem_max - fixed) / 16);
+        if (Db > cap) {
+            n_win = (int)((Db + cap - 1) / cap);
+            win = (((Db + n_win - 1) / n_win) + 7) & ~i64(7);
+        }
+    } else win = 0;
+    R->win_cols = (int)win;
+    R->n_win = n_win;
+    R->smem = fixed + (size_t)win * 16;
+    // threads / columns per thread: small rows -> several blocks per SM; big rows -> 1024 threads
+    int threads, cpt;
+    if (R->smem > 110 * 1024) threads = 1024;
+    else if (R->smem > 56 * 1024) threads = 512;
+    else threads = 256;
+    const i64 per_block_max = (i64)threads * 4;
+    int n_chunks = (int)((Db + per_block_max - 1) / per_block_max);
+    i64 chunk = ((Db + n_chunks - 1) / n_chunks + 31) & ~i64(31);
+    cpt = (int)((chunk + threads - 1) / threads);
+    while (threads > 64 && chunk <= threads / 2) threads /= 2;  // tiny rows
+    cpt = (int)((chunk + threads - 1) / threads);
+    R->threads = threads;
+    R->cpt = cpt <= 1 ? 1 : (cpt <= 2 ? 2 : 4);
+    R->n_chunks = n_chunks;
+    R->chunk_cols = (int)chunk;
+    R->tstride = (i64)R->n_chunks * R->threads * R->cpt;
+    BS_REQUIRE((double)R->n_tkeys * (double)R->tstride * 2.0 <= 8e9, BS_ERR_ALLOC, "row plan: column tables too large");
+    BS_REQUIRE(max_keys <= 2048, BS_ERR_ARG, "row plan: too many keys under one alpha mask");
+    BS_CUDA(R->d_xa.upload(xa_list, st));
+    BS_CUDA(R->d_xa_hdr.upload(hdrs, st));
+    BS_CUDA(R->d_items.upload(items, st));
+    BS_CUDA(R->d_key_dz.upload(key_dz, st));
+    BS_CUDA(R->d_key_s0.upload(key_s0, st));
+    BS_CUDA(R->d_s_za.upload(s_za, st));
+    BS_CUDA(R->d_s_w.upload(s_w, st));
+    DevBuf<uint2> d_tkeys;
+    BS_CUDA(d_tkeys.upload(tkeys, st));
+    BS_CUDA(R->d_ttab.alloc((size_t)std::max<i64>(1, R->n_tkeys) * R->tstride));
+    for (i64 k0 = 0; k0 < R->n_tkeys; k0 += 32768) {
+        dim3 grid((unsigned)((R->tstride + 255) / 256), (unsigned)std::min<i64>(32768, R->n_tkeys - k0));
+        k_fill_ttab<<<grid, 256, 0, st>>>(B, d_tkeys.p + k0, R->tstride, R->threads, R->cpt, R->chunk_cols,
+                                          R->d_ttab.p + k0 * R->tstride);
+        BS_COUNT_LAUNCH(1);
+    }
+    // per-row valid alpha masks
+    DevBuf<int> cnt;
+    BS_CUDA(cnt.alloc(Da));
+    BS_CUDA(R->d_row_off.alloc(Da + 1));
+    const unsigned nb = (unsigned)((Da + 127) / 128);
+    k_row_count2<<<nb, 128, 0, st>>>(A, R->d_xa.p, R->n_xa, cnt.p);
+    std::vector<int> hcnt(Da);
+    BS_CUDA(cudaMemcpyAsync(hcnt.data(), cnt.p, Da * 4, cudaMemcpyDeviceToHost, st));
+    BS_CUDA(cudaStreamSynchronize(st));
+    std::vector<i64> hoff(Da + 1, 0);
+    for (i64 r = 0; r < Da; ++r) hoff[r + 1] = hoff[r] + hcnt[r];
+    R->n_row_ent = hoff[Da];
+    BS_CUDA(cudaMemcpyAsync(R->d_row_off.p, hoff.data(), (Da + 1) * 8, cudaMemcpyHostToDevice, st));
+    BS_CUDA(R->d_row_ent.alloc(std::max<i64>(1, R->n_row_ent)));
+    k_row_fill2<<<nb, 128, 0, st>>>(A, R->d_xa.p, R->n_xa, R->d_row_off.p, R->d_row_ent.p);
+    BS_COUNT_LAUNCH(2);
+    BS_CUDA(cudaGetLastError());
+    BS_CUDA(cudaStreamSynchronize(st));  // host vectors go out of scope
+
+    RowPlanDev& d = R->dev;
+    d.A = A;
+    d.B = B;
+    d.row_off = R->d_row_off.p;
+    d.row_ent = R->d_row_ent.p;
+    d.xa_hdr = R->d_xa_hdr.p;
+    d.items = R->d_items.p;
+    d.key_dz = R->d_key_dz.p;
+    d.key_s0 = R->d_key_s0.p;
+    d.s_za = R->d_s_za.p;
+    d.s_w = R->d_s_w.p;
+    d.ttab = R->d_ttab.p;
+    d.tstride = R->tstride;
+    d.max_keys = std::max(max_keys, 1);
+    d.win_cols = R->win_cols;
+    d.n_win = R->n_win;
+    d.chunk_cols = R->chunk_cols;
+    return BS_OK;
+}

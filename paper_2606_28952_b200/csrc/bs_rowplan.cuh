@@ -1,0 +1,71 @@
+// v2 "row plan": sector-specific tables of one (operator, sector) pair for the row kernel
+// (bs_rowkernel.cu).  See DESIGN.md "Apply kernel v2".
+//
+// Groups are split by (xa, xb) = (alpha part, beta part) of their X mask (Eq. 28):
+//   D  xa = 0, xb = 0   diagonal
+//   B  xa = 0, xb != 0  source in the same row, another column
+//   A  xa != 0, xb = 0  source in another row, same column (coalesced, no gather)
+//   AB both             source in another row, another column
+// Phase factorisation: within a group, strings are bucketed by their beta Z
+// mask ("keys"): F_g(ta, tb) = sum_j V_gj(ta) (-1)^{popc(zb_gj & tb)},
+// V_gj(ta) = sum_{k: zb_k = zb_gj} w_k (-1)^{popc(za_k & ta)}.  V is evaluated once per (row, group)
+// into shared memory; the per-target work is one term per KEY, not per string.
+// Column tables: for every distinct (xb, zb_g0) pair a u16 table T[col] = source column | sign << 15
+// (0xFFFF: tb ^ xb leaves the sector) replaces the per-target validity test, rank and first POPC.
+#pragma once
+#include "bs_internal.cuh"
+
+constexpr u32 kTkeyIdent = 0xFFFFFFFFu;  // xb = 0 and zb_g0 = 0: source column = target column, sign +
+
+struct __align__(16) XaHdr {
+    u32 item0, item1;  // items (groups) under this alpha mask
+    u32 key0, key1;    // their keys, contiguous: V slot of key k is k - key0
+    u32 stage;         // 1: some item has xb != 0 -> the source row is staged in shared memory
+    u32 pad[3];
+};
+struct __align__(16) RowItem {
+    u32 tkey;   // column table id or kTkeyIdent
+    u32 key0;   // first key (global index)
+    u32 nkeys;  // >= 1
+    u32 single; // 1: every dz of keys 1.. has exactly one bit (bit test instead of POPC)
+};
+
+// device view handed to the kernel by value
+struct RowPlanDev {
+    SpinTab A, B;               // row strings (A) and column strings (B); swapped in the transposed plan
+    const i64* row_off;         // [Da + 1]
+    const uint2* row_ent;       // {xa id, source row}
+    const XaHdr* xa_hdr;
+    const RowItem* items;
+    const u32* key_dz;          // [n_keys] zb_key ^ zb_g0
+    const u32* key_s0;          // [n_keys + 1] string range of each key
+    const u32* s_za;            // [n_strings]
+    const double2* s_w;         // [n_strings]
+    const unsigned short* ttab; // [n_tkeys][tstride], thread-blocked: slot (chunk*threads + tid)*cpt + c holds
+                                // column chunk*chunk_cols + tid + c*threads (0xFFFF beyond the chunk / row)
+    i64 tstride;
+    int max_keys;               // max keys under one alpha mask (V slots in shared memory)
+    int win_cols;               // columns of a source row staged at once (>= Db: whole row)
+    int n_win;                  // number of windows
+    int chunk_cols;             // target columns per thread block
+};
+
+struct bs_rowplan {
+    bool real_w = true;
+    i64 n_items = 0, n_keys = 0, n_strings = 0, n_tkeys = 0, n_row_ent = 0;
+    int n_xa = 0, max_keys = 0;
+    bool any_stage = false;
+    DevBuf<u32> d_xa;
+    DevBuf<XaHdr> d_xa_hdr;
+    DevBuf<RowItem> d_items;
+    DevBuf<u32> d_key_dz, d_key_s0, d_s_za;
+    DevBuf<double2> d_s_w;
+    DevBuf<unsigned short> d_ttab;
+    DevBuf<i64> d_row_off;
+    DevBuf<uint2> d_row_ent;
+    i64 tstride = 0;
+    // launch geometry
+    int threads = 256, cpt = 1, n_chunks = 1, chunk_cols = 0, win_cols = 0, n_win = 1;
+    size_t smem = 0;
+    RowPlanDev dev{};
+};
