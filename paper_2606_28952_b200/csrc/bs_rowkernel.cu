@@ -75,7 +75,7 @@ __device__ __forceinline__ void load_entries(const unsigned short* __restrict__ 
 
 // sum over the remaining keys of a multi-key group: f += sum_j (+-) V_j, sign from the column string
 template <bool REALW>
-__device__ __forceinline__ typename VT<REALW>::type multi_key(typename VT<REALW>::type f,
+__device__ __noinline__ typename VT<REALW>::type multi_key(typename VT<REALW>::type f,
                                                               const typename VT<REALW>::type* __restrict__ v,
                                                               const u32* __restrict__ dz, u32 nkeys, u32 single, u32 tb) {
     using V = VT<REALW>;
@@ -87,8 +87,66 @@ __device__ __forceinline__ typename VT<REALW>::type multi_key(typename VT<REALW>
     return f;
 }
 
+// All items of one row entry (one valid alpha mask) for this thread's CPT columns.
+// STAGED: the source row (window [w0, w0 + wn)) is in shared memory; else it is read from global memory
+// (only x_b = 0 items then, i.e. source column = target column).
+template <bool REALW, int CPT, bool STAGED, bool WINDOWED>
+__device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* __restrict__ items4, u32 item0, u32 item1,
+                                              u32 hkey0, const typename VT<REALW>::type* __restrict__ vbase,
+                                              const double2* __restrict__ srow, const double2* __restrict__ srcp,
+                                              u32 w0, u32 wn, u32 tpos, const u32 (&col)[CPT], const u32 (&tb)[CPT],
+                                              double2 (&acc)[CPT]) {
+    using V = VT<REALW>;
+    using vt = typename V::type;
+    uint4 nxt = __ldg(items4 + item0);
+    for (u32 i = item0; i < item1; ++i) {
+        const uint4 it = nxt;  // {tkey, key0, nkeys, single}
+        if (i + 1 < item1) nxt = __ldg(items4 + i + 1);
+        const vt* __restrict__ v = vbase + (it.y - hkey0);
+        const vt f0 = v[0];
+        if (it.x == kTkeyIdent) {
+            // x_b = 0, no beta sign on the first key: same column of the source row
+            double2 a[CPT];
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) {
+                if (STAGED) a[c] = (!WINDOWED || (col[c] - w0) < wn) ? srow[col[c] - w0] : make_double2(0.0, 0.0);
+                else a[c] = __ldg(srcp + col[c]);
+            }
+            if (it.z == 1) {
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) V::fma(acc[c], f0, 0u, a[c]);
+            } else {
+#pragma unroll
+                for (int c = 0; c < CPT; ++c)
+                    V::fma(acc[c], multi_key<REALW>(f0, v, P.key_dz + it.y, it.z, it.w, tb[c]), 0u, a[c]);
+            }
+        } else {
+            u32 en16[CPT];
+            load_entries<CPT>(P.ttab + (i64)it.x * P.tstride + tpos, en16);
+            if (it.z == 1) {
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) {
+                    const u32 src = en16[c] & 0x7FFFu;
+                    if (en16[c] == 0xFFFFu || (WINDOWED && (src - w0) >= wn)) continue;
+                    const double2 a = STAGED ? srow[src - w0] : __ldg(srcp + src);
+                    V::fma(acc[c], f0, en16[c] >> 15, a);
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) {
+                    const u32 src = en16[c] & 0x7FFFu;
+                    if (en16[c] == 0xFFFFu || (WINDOWED && (src - w0) >= wn)) continue;
+                    const vt f = multi_key<REALW>(f0, v, P.key_dz + it.y, it.z, it.w, tb[c]);
+                    const double2 a = STAGED ? srow[src - w0] : __ldg(srcp + src);
+                    V::fma(acc[c], f, en16[c] >> 15, a);
+                }
+            }
+        }
+    }
+}
+
 template <int MODE, bool REALW, int CPT, int MAXT>
-__global__ void __launch_bounds__(MAXT)
+__global__ void __launch_bounds__(MAXT, (MAXT == 1024 ? 1 : (MAXT == 512 ? 2 : 4)))
 k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict__ out, i64 row_lo, i64 col_lo,
        i64 col_hi, int chunk0, Epilogue ep, double2* __restrict__ partials) {
     using V = VT<REALW>;
@@ -122,15 +180,26 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
     }
     u32 phase = 0;
     const uint4* __restrict__ items4 = reinterpret_cast<const uint4*>(P.items);
+    const int warp = tid >> 5, lane = tid & 31, nwarps = nt >> 5;
+    const u32 vcap = (u32)P.max_keys;
     const i64 e0 = P.row_off[row], e1 = P.row_off[row + 1];
-    for (i64 e = e0; e < e1; ++e) {
-        const uint2 ent = __ldg(P.row_ent + e);
-        const uint4 h4 = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + ent.x));      // item0,item1,key0,key1
-        const u32 stage = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + ent.x) + 4);
-        const u32 item0 = h4.x, item1 = h4.y, key0 = h4.z, key1 = h4.w;
-        const double2* __restrict__ srcp = psi + (i64)ent.y * Db;
+    i64 e = e0;
+    while (e < e1) {
+        // ---- batch: one staged entry, or a run of non-staged entries whose keys fit the V slots ---------
+        const uint4 first = __ldg(P.row_ent + e);
+        const u32 stage = first.w >> 31;
+        const u32 kbase = first.z;
+        i64 be = e + 1;
+        if (!stage) {
+            while (be < e1) {
+                const uint4 nx = __ldg(P.row_ent + be);
+                if ((nx.w >> 31) || nx.z + (nx.w & 0x7FFFFFFFu) - kbase > vcap) break;
+                ++be;
+            }
+        }
+        const double2* __restrict__ srow_g = psi + (i64)first.y * Db;  // staged batches have one entry
+        __syncthreads();  // everyone is done with the previous batch's V slots and staged row
         const int n_win = stage ? P.n_win : 1;
-        __syncthreads();  // everyone is done with the previous entry's V slots and staged row
         for (int w = 0; w < n_win; ++w) {
             const u32 w0 = (u32)w * (u32)P.win_cols;
             const u32 wn = stage ? min((u32)P.win_cols, Db - w0) : 0u;
@@ -141,17 +210,23 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                     mbar_expect_tx(bar, bytes);
                     for (u32 o = 0; o < bytes; o += 32768u)
                         tma_bulk_g2s(reinterpret_cast<unsigned char*>(srow) + o,
-                                     reinterpret_cast<const unsigned char*>(srcp + w0) + o, min(32768u, bytes - o), bar);
+                                     reinterpret_cast<const unsigned char*>(srow_g + w0) + o, min(32768u, bytes - o),
+                                     bar);
                 }
             }
             if (w == 0) {
-                // phase factors of every key under this alpha mask (overlaps the bulk copy)
-                for (u32 k = key0 + tid; k < key1; k += nt) {
-                    vt f = V::zero();
-                    const u32 s1 = __ldg(P.key_s0 + k + 1);
-                    for (u32 s = __ldg(P.key_s0 + k); s < s1; ++s)
-                        V::addflip(f, V::from(__ldg(P.s_w + s)), (u32)__popc(__ldg(P.s_za + s) & ta) & 1u);
-                    sV[k - key0] = f;
+                // phase factors of every key of the batch, one warp per entry (overlaps the bulk copy)
+                for (i64 j = e + warp; j < be; j += nwarps) {
+                    const uint4 en = __ldg(P.row_ent + j);
+                    const u32 key0 = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + en.x) + 2);
+                    const u32 nk = en.w & 0x7FFFFFFFu;
+                    for (u32 k = lane; k < nk; k += 32) {
+                        vt f = V::zero();
+                        const u32 s1 = __ldg(P.key_s0 + key0 + k + 1);
+                        for (u32 s = __ldg(P.key_s0 + key0 + k); s < s1; ++s)
+                            V::addflip(f, V::from(__ldg(P.s_w + s)), (u32)__popc(__ldg(P.s_za + s) & ta) & 1u);
+                        sV[en.z - kbase + k] = f;
+                    }
                 }
                 __syncthreads();
             }
@@ -159,38 +234,23 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                 mbar_wait(bar, phase);
                 phase ^= 1u;
             }
-            const bool windowed = stage && n_win > 1;
-            uint4 nxt = item0 < item1 ? __ldg(items4 + item0) : make_uint4(0, 0, 0, 0);
-            for (u32 i = item0; i < item1; ++i) {
-                const uint4 it = nxt;  // {tkey, key0, nkeys, single}
-                if (i + 1 < item1) nxt = __ldg(items4 + i + 1);
-                const vt* __restrict__ v = sV + (it.y - key0);
-                const vt f0 = v[0];
-                if (it.x == kTkeyIdent) {
-                    // x_b = 0, no beta sign on the first key: same column of the source row
-#pragma unroll
-                    for (int c = 0; c < CPT; ++c) {
-                        if (windowed && (col[c] - w0) >= wn) continue;
-                        vt f = f0;
-                        if (it.z > 1) f = multi_key<REALW>(f, v, P.key_dz + it.y, it.z, it.w, tb[c]);
-                        const double2 a = stage ? srow[col[c] - w0] : __ldg(srcp + col[c]);
-                        V::fma(acc[c], f, 0u, a);
-                    }
-                } else {
-                    u32 en[CPT];
-                    load_entries<CPT>(P.ttab + (i64)it.x * P.tstride + tpos, en);
-#pragma unroll
-                    for (int c = 0; c < CPT; ++c) {
-                        const u32 src = en[c] & 0x7FFFu;
-                        if (en[c] == 0xFFFFu || (windowed && (src - w0) >= wn)) continue;
-                        vt f = f0;
-                        if (it.z > 1) f = multi_key<REALW>(f, v, P.key_dz + it.y, it.z, it.w, tb[c]);
-                        const double2 a = stage ? srow[src - w0] : __ldg(srcp + src);
-                        V::fma(acc[c], f, en[c] >> 15, a);
-                    }
-                }
+            for (i64 j = e; j < be; ++j) {
+                const uint4 en = __ldg(P.row_ent + j);
+                const uint4 h4 = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + en.x));  // item0,item1,key0,key1
+                const double2* __restrict__ srcp = psi + (i64)en.y * Db;
+                const vt* __restrict__ vbase = sV + (en.z - kbase);
+                if (!stage)
+                    process_entry<REALW, CPT, false, false>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, 0u, 0u, tpos,
+                                                            col, tb, acc);
+                else if (n_win == 1)
+                    process_entry<REALW, CPT, true, false>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, 0u, wn, tpos,
+                                                           col, tb, acc);
+                else
+                    process_entry<REALW, CPT, true, true>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, w0, wn, tpos,
+                                                          col, tb, acc);
             }
         }
+        e = be;
     }
     double2 dot = make_double2(0.0, 0.0);
 #pragma unroll
@@ -262,8 +322,13 @@ k_transpose_add_finish(const double2* raw, const double2* __restrict__ out_t,
 template <int MODE, bool REALW, int CPT>
 cudaError_t launch_k_rows_t(const bs_rowplan* R, dim3 grid, cudaStream_t st, const double2* psi, double2* out,
                             i64 row_lo, i64 col_lo, i64 col_hi, int chunk0, const Epilogue& ep, double2* partials) {
-    if (R->threads > 256) {
+    if (R->threads > 512) {
         auto k = k_rows<MODE, REALW, CPT, 1024>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
+    } else if (R->threads > 256) {
+        auto k = k_rows<MODE, REALW, CPT, 512>;
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
         if (e != cudaSuccess) return e;
         k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
@@ -284,8 +349,8 @@ cudaError_t launch_k_rows(const bs_rowplan* R, cudaStream_t st, const double2* p
     dim3 grid((unsigned)(row_hi - row_lo), n_chunks);
     BS_COUNT_LAUNCH(1);
 #define BS_ROWS(RW, C) launch_k_rows_t<MODE, RW, C>(R, grid, st, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials)
-    if (R->real_w) return R->cpt == 1 ? BS_ROWS(true, 1) : (R->cpt == 2 ? BS_ROWS(true, 2) : BS_ROWS(true, 4));
-    return R->cpt == 1 ? BS_ROWS(false, 1) : (R->cpt == 2 ? BS_ROWS(false, 2) : BS_ROWS(false, 4));
+    if (R->real_w) return R->cpt == 1 ? BS_ROWS(true, 1) : BS_ROWS(true, 4);
+    return R->cpt == 1 ? BS_ROWS(false, 1) : BS_ROWS(false, 4);
 #undef BS_ROWS
 }
 

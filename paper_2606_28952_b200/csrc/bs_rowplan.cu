@@ -43,15 +43,20 @@ __global__ void k_row_count2(SpinTab A, const u32* __restrict__ xa, int n_xa, in
     cnt[r] = c;
 }
 
-__global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, int n_xa, const i64* __restrict__ off,
-                            uint2* __restrict__ ent) {
+__global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* __restrict__ hdr, int n_xa,
+                            const i64* __restrict__ off, uint4* __restrict__ ent) {
     i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (r >= A.D) return;
     u32 ta = A.str[r];
     i64 o = off[r];
+    u32 koff = 0;
     for (int i = 0; i < n_xa; ++i) {
         u32 m = __ldg(xa + i);
-        if (2 * __popc(ta & m) == __popc(m)) ent[o++] = make_uint2((u32)i, spin_rank(A, ta ^ m));
+        if (2 * __popc(ta & m) == __popc(m)) {
+            const u32 nk = hdr[i].key1 - hdr[i].key0;
+            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31));
+            koff += nk;
+        }
     }
 }
 
@@ -134,7 +139,8 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     R->any_stage = any_stage;
     // ---- launch geometry ---------------------------------------------------------------------
     // Shared memory: [mbarrier 16 B][V slots: max_keys * 16 B][row window: win_cols * 16 B].
-    const size_t fixed = 16 + (size_t)std::max(max_keys, 1) * 16;
+    const int vcap = std::max(max_keys, 512);
+    const size_t fixed = 16 + (size_t)vcap * 16;
     const size_t smem_max = 227 * 1024 - 1024;
     i64 win = Db;
     int n_win = 1;
@@ -151,7 +157,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     // threads / columns per thread: small rows -> several blocks per SM; big rows -> 1024 threads
     int threads, cpt;
     if (R->smem > 110 * 1024) threads = 1024;
-    else if (R->smem > 56 * 1024) threads = 512;
+    else if (R->smem > 56 * 1024 || Db >= 2048) threads = 512;
     else threads = 256;
     const i64 per_block_max = (i64)threads * 4;
     int n_chunks = (int)((Db + per_block_max - 1) / per_block_max);
@@ -160,7 +166,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     while (threads > 64 && chunk <= threads / 2) threads /= 2;  // tiny rows
     cpt = (int)((chunk + threads - 1) / threads);
     R->threads = threads;
-    R->cpt = cpt <= 1 ? 1 : (cpt <= 2 ? 2 : 4);
+    R->cpt = cpt <= 1 ? 1 : 4;
     R->n_chunks = n_chunks;
     R->chunk_cols = (int)chunk;
     R->tstride = (i64)R->n_chunks * R->threads * R->cpt;
@@ -196,7 +202,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     R->n_row_ent = hoff[Da];
     BS_CUDA(cudaMemcpyAsync(R->d_row_off.p, hoff.data(), (Da + 1) * 8, cudaMemcpyHostToDevice, st));
     BS_CUDA(R->d_row_ent.alloc(std::max<i64>(1, R->n_row_ent)));
-    k_row_fill2<<<nb, 128, 0, st>>>(A, R->d_xa.p, R->n_xa, R->d_row_off.p, R->d_row_ent.p);
+    k_row_fill2<<<nb, 128, 0, st>>>(A, R->d_xa.p, R->d_xa_hdr.p, R->n_xa, R->d_row_off.p, R->d_row_ent.p);
     BS_COUNT_LAUNCH(2);
     BS_CUDA(cudaGetLastError());
     BS_CUDA(cudaStreamSynchronize(st));  // host vectors go out of scope
@@ -214,7 +220,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     d.s_w = R->d_s_w.p;
     d.ttab = R->d_ttab.p;
     d.tstride = R->tstride;
-    d.max_keys = std::max(max_keys, 1);
+    d.max_keys = vcap;
     d.win_cols = R->win_cols;
     d.n_win = R->n_win;
     d.chunk_cols = R->chunk_cols;

@@ -34,7 +34,8 @@ struct __align__(16) RowItem {
 struct RowPlanDev {
     SpinTab A, B;               // row strings (A) and column strings (B); swapped in the transposed plan
     const i64* row_off;         // [Da + 1]
-    const uint2* row_ent;       // {xa id, source row}
+    const uint4* row_ent;       // {xa id, source row, V-slot offset within the row (prefix sum of key counts),
+                                //  key count | stage << 31}
     const XaHdr* xa_hdr;
     const RowItem* items;
     const u32* key_dz;          // [n_keys] zb_key ^ zb_g0
@@ -44,7 +45,7 @@ struct RowPlanDev {
     const unsigned short* ttab; // [n_tkeys][tstride], thread-blocked: slot (chunk*threads + tid)*cpt + c holds
                                 // column chunk*chunk_cols + tid + c*threads (0xFFFF beyond the chunk / row)
     i64 tstride;
-    int max_keys;               // max keys under one alpha mask (V slots in shared memory)
+    int max_keys;               // V slots in shared memory (>= max keys under one alpha mask)
     int win_cols;               // columns of a source row staged at once (>= Db: whole row)
     int n_win;                  // number of windows
     int chunk_cols;             // target columns per thread block
@@ -62,7 +63,7 @@ struct bs_rowplan {
     DevBuf<double2> d_s_w;
     DevBuf<unsigned short> d_ttab;
     DevBuf<i64> d_row_off;
-    DevBuf<uint2> d_row_ent;
+    DevBuf<uint4> d_row_ent;
     i64 tstride = 0;
     // launch geometry
     int threads = 256, cpt = 1, n_chunks = 1, chunk_cols = 0, win_cols = 0, n_win = 1;
