@@ -73,18 +73,29 @@ __device__ __forceinline__ void load_entries(const unsigned short* __restrict__ 
     }
 }
 
-// sum over the remaining keys of a multi-key group: f += sum_j (+-) V_j, sign from the column string
-template <bool REALW>
-__device__ __noinline__ typename VT<REALW>::type multi_key(typename VT<REALW>::type f,
-                                                              const typename VT<REALW>::type* __restrict__ v,
-                                                              const u32* __restrict__ dz, u32 nkeys, u32 single, u32 tb) {
+// Remaining keys of a multi-key group for all CPT columns of the thread at once:
+// f[c] = v[0] + sum_{j>=1} (+-) v[j], sign = parity(dz_j & tb[c]).  Single-bit dz (the common case: Z on one
+// beta orbital) needs no POPC: the tested bit is shifted into the sign position of the high word.
+template <bool REALW, int CPT>
+__device__ __forceinline__ void multi_key(typename VT<REALW>::type (&f)[CPT],
+                                          const typename VT<REALW>::type* __restrict__ v,
+                                          const u32* __restrict__ dz, u32 nkeys, u32 single, const u32 (&tb)[CPT]) {
     using V = VT<REALW>;
     if (single) {
-        for (u32 j = 1; j < nkeys; ++j) V::addflip(f, v[j], (tb & __ldg(dz + j)) ? 1u : 0u);
+        for (u32 j = 1; j < nkeys; ++j) {
+            const int sh = __clz((int)__ldg(dz + j));
+            const typename V::type vj = v[j];
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) V::addflip(f[c], vj, (tb[c] << sh) >> 31);
+        }
     } else {
-        for (u32 j = 1; j < nkeys; ++j) V::addflip(f, v[j], (u32)__popc(tb & __ldg(dz + j)) & 1u);
+        for (u32 j = 1; j < nkeys; ++j) {
+            const u32 m = __ldg(dz + j);
+            const typename V::type vj = v[j];
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) V::addflip(f[c], vj, (u32)__popc(tb[c] & m) & 1u);
+        }
     }
-    return f;
 }
 
 // All items of one row entry (one valid alpha mask) for this thread's CPT columns.
@@ -116,9 +127,12 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) V::fma(acc[c], f0, 0u, a[c]);
             } else {
+                vt f[CPT];
 #pragma unroll
-                for (int c = 0; c < CPT; ++c)
-                    V::fma(acc[c], multi_key<REALW>(f0, v, P.key_dz + it.y, it.z, it.w, tb[c]), 0u, a[c]);
+                for (int c = 0; c < CPT; ++c) f[c] = f0;
+                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w, tb);
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) V::fma(acc[c], f[c], 0u, a[c]);
             }
         } else {
             u32 en16[CPT];
@@ -132,13 +146,16 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
                     V::fma(acc[c], f0, en16[c] >> 15, a);
                 }
             } else {
+                vt f[CPT];
+#pragma unroll
+                for (int c = 0; c < CPT; ++c) f[c] = f0;
+                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w, tb);
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) {
                     const u32 src = en16[c] & 0x7FFFu;
                     if (en16[c] == 0xFFFFu || (WINDOWED && (src - w0) >= wn)) continue;
-                    const vt f = multi_key<REALW>(f0, v, P.key_dz + it.y, it.z, it.w, tb[c]);
                     const double2 a = STAGED ? srow[src - w0] : __ldg(srcp + src);
-                    V::fma(acc[c], f, en16[c] >> 15, a);
+                    V::fma(acc[c], f[c], en16[c] >> 15, a);
                 }
             }
         }
@@ -193,7 +210,7 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
         if (!stage) {
             while (be < e1) {
                 const uint4 nx = __ldg(P.row_ent + be);
-                if ((nx.w >> 31) || nx.z + (nx.w & 0x7FFFFFFFu) - kbase > vcap) break;
+                if ((nx.w >> 31) || nx.z + (nx.w & 0x3FFFFFFFu) - kbase > vcap) break;
                 ++be;
             }
         }
@@ -219,7 +236,7 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                 for (i64 j = e + warp; j < be; j += nwarps) {
                     const uint4 en = __ldg(P.row_ent + j);
                     const u32 key0 = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + en.x) + 2);
-                    const u32 nk = en.w & 0x7FFFFFFFu;
+                    const u32 nk = en.w & 0x3FFFFFFFu;
                     for (u32 k = lane; k < nk; k += 32) {
                         vt f = V::zero();
                         const u32 s1 = __ldg(P.key_s0 + key0 + k + 1);
@@ -236,9 +253,19 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
             }
             for (i64 j = e; j < be; ++j) {
                 const uint4 en = __ldg(P.row_ent + j);
-                const uint4 h4 = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + en.x));  // item0,item1,key0,key1
                 const double2* __restrict__ srcp = psi + (i64)en.y * Db;
                 const vt* __restrict__ vbase = sV + (en.z - kbase);
+                if (en.w & 0x40000000u) {
+                    // "simple" entry: one group, x_b = 0, one key: out[row, :] += V * psi[source row, :]
+                    const vt f0 = vbase[0];
+                    double2 a[CPT];
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) a[c] = __ldg(srcp + col[c]);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) V::fma(acc[c], f0, 0u, a[c]);
+                    continue;
+                }
+                const uint4 h4 = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + en.x));  // item0,item1,key0,key1
                 if (!stage)
                     process_entry<REALW, CPT, false, false>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, 0u, 0u, tpos,
                                                             col, tb, acc);

@@ -54,7 +54,7 @@ __global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* 
         u32 m = __ldg(xa + i);
         if (2 * __popc(ta & m) == __popc(m)) {
             const u32 nk = hdr[i].key1 - hdr[i].key0;
-            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31));
+            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31) | (hdr[i].pad[0] << 30));
             koff += nk;
         }
     }
@@ -124,6 +124,11 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
         hdrs.back().key1 = (u32)key_dz.size();
     }
     key_s0.push_back((u32)s_za.size());
+    // "simple" alpha masks: one group with x_b = 0, no beta sign and a single key (pad[0] = 1)
+    for (auto& h : hdrs) {
+        const RowItem& it = items[h.item0];
+        h.pad[0] = (h.item1 - h.item0 == 1 && !h.stage && it.tkey == kTkeyIdent && it.nkeys == 1) ? 1u : 0u;
+    }
     bool any_stage = false;
     for (auto& h : hdrs) {
         max_keys = std::max(max_keys, (int)(h.key1 - h.key0));
