@@ -162,6 +162,42 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
     }
 }
 
+// Column-list pass of a staged entry: every single-key x_b != 0 group under the alpha mask, compacted per
+// column (no invalid lanes, no branches): entry = source column | sign << 15 | table id << 16, V from sVx[id].
+template <bool REALW, int CPT, bool WINDOWED>
+__device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT<REALW>::type* __restrict__ sVx,
+                                          const double2* __restrict__ srow, u32 w0, u32 wn, u32 tpos,
+                                          double2 (&acc)[CPT]) {
+    using V = VT<REALW>;
+    const u32* __restrict__ L = P.ltab + tpos;
+    u32 en[CPT], nx[CPT];
+    auto load = [&](int j, u32 (&e)[CPT]) {
+        const u32* p = L + (i64)j * P.tstride;
+        if (CPT == 4) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+            e[0] = v.x;
+            e[1 % CPT] = v.y;
+            e[2 % CPT] = v.z;
+            e[3 % CPT] = v.w;
+        } else {
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) e[c] = __ldg(p + c);
+        }
+    };
+    load(0, nx);
+    for (int j = 0; j < P.l_max; ++j) {
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) en[c] = nx[c];
+        if (j + 1 < P.l_max) load(j + 1, nx);
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) {
+            const u32 src = en[c] & 0x7FFFu;
+            if (WINDOWED && (src - w0) >= wn) continue;
+            V::fma(acc[c], sVx[en[c] >> 16], (en[c] >> 15) & 1u, srow[src - w0]);
+        }
+    }
+}
+
 template <int MODE, bool REALW, int CPT, int MAXT>
 __global__ void __launch_bounds__(MAXT, (MAXT == 1024 ? 1 : (MAXT == 512 ? 2 : 4)))
 k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict__ out, i64 row_lo, i64 col_lo,
@@ -172,7 +208,8 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
     __shared__ double2 sh_red[32];
     u64* bar = reinterpret_cast<u64*>(smem_raw);
     vt* sV = reinterpret_cast<vt*>(smem_raw + 16);
-    double2* srow = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)P.max_keys * 16);
+    vt* sVx = reinterpret_cast<vt*>(smem_raw + 16 + (size_t)P.max_keys * 16);
+    double2* srow = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)(P.max_keys + P.n_listed + 1) * 16);
     const int tid = threadIdx.x, nt = blockDim.x;
     const i64 row = row_lo + blockIdx.x;
     const u32 Db = (u32)P.B.D;
@@ -215,7 +252,14 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
             }
         }
         const double2* __restrict__ srow_g = psi + (i64)first.y * Db;  // staged batches have one entry
+        const uint4 hs = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + first.x) + 1);  // stage,simple,item_split,key_split
+        const u32 item_end = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + first.x) + 1);
+        const bool listed = stage && hs.z < item_end;
         __syncthreads();  // everyone is done with the previous batch's V slots and staged row
+        if (listed) {
+            for (int k = tid; k <= P.n_listed; k += nt) sVx[k] = V::zero();
+            __syncthreads();
+        }
         const int n_win = stage ? P.n_win : 1;
         for (int w = 0; w < n_win; ++w) {
             const u32 w0 = (u32)w * (u32)P.win_cols;
@@ -243,6 +287,7 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                         for (u32 s = __ldg(P.key_s0 + key0 + k); s < s1; ++s)
                             V::addflip(f, V::from(__ldg(P.s_w + s)), (u32)__popc(__ldg(P.s_za + s) & ta) & 1u);
                         sV[en.z - kbase + k] = f;
+                        if (listed && key0 + k >= hs.w) sVx[__ldg(&P.items[hs.z + (key0 + k - hs.w)].tkey)] = f;
                     }
                 }
                 __syncthreads();
@@ -269,12 +314,17 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                 if (!stage)
                     process_entry<REALW, CPT, false, false>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, 0u, 0u, tpos,
                                                             col, tb, acc);
-                else if (n_win == 1)
-                    process_entry<REALW, CPT, true, false>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, 0u, wn, tpos,
-                                                           col, tb, acc);
-                else
-                    process_entry<REALW, CPT, true, true>(P, items4, h4.x, h4.y, h4.z, vbase, srow, srcp, w0, wn, tpos,
-                                                          col, tb, acc);
+                else if (n_win == 1) {
+                    if (h4.x < hs.z)
+                        process_entry<REALW, CPT, true, false>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, 0u, wn,
+                                                               tpos, col, tb, acc);
+                    if (listed) list_pass<REALW, CPT, false>(P, sVx, srow, 0u, wn, tpos, acc);
+                } else {
+                    if (h4.x < hs.z)
+                        process_entry<REALW, CPT, true, true>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, w0, wn,
+                                                              tpos, col, tb, acc);
+                    if (listed) list_pass<REALW, CPT, true>(P, sVx, srow, w0, wn, tpos, acc);
+                }
             }
         }
         e = be;

@@ -31,6 +31,22 @@ __global__ void k_fill_ttab(SpinTab B, const uint2* __restrict__ keys, i64 tstri
     T[(i64)blockIdx.y * tstride + slot] = e;
 }
 
+// l_max == 0: count the valid listed tables of every slot; else write the padded list
+__global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, int n_listed, int l_max,
+                             u32* __restrict__ L, int* __restrict__ cnt) {
+    const i64 slot = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (slot >= tstride) return;
+    int j = 0;
+    for (int t = 0; t < n_listed; ++t) {
+        const u32 e = T[(i64)t * tstride + slot];
+        if (e == 0xFFFFu) continue;
+        if (l_max) L[(i64)j * tstride + slot] = e | ((u32)t << 16);
+        ++j;
+    }
+    if (!l_max) cnt[slot] = j;
+    else for (; j < l_max; ++j) L[(i64)j * tstride + slot] = (u32)n_listed << 16;
+}
+
 __global__ void k_row_count2(SpinTab A, const u32* __restrict__ xa, int n_xa, int* __restrict__ cnt) {
     i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (r >= A.D) return;
@@ -54,7 +70,7 @@ __global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* 
         u32 m = __ldg(xa + i);
         if (2 * __popc(ta & m) == __popc(m)) {
             const u32 nk = hdr[i].key1 - hdr[i].key0;
-            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31) | (hdr[i].pad[0] << 30));
+            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31) | (hdr[i].simple << 30));
             koff += nk;
         }
     }
@@ -63,16 +79,45 @@ __global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* 
 }  // namespace
 
 // groups: already z-reduced, oriented (xa = row-spin mask, xb = column-spin mask), sorted by (xa, xb).
-int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const SpinTab& A, const SpinTab& B,
+int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, const SpinTab& A, const SpinTab& B,
                      cudaStream_t st) {
     const i64 Da = A.D, Db = B.D;
+    // ---- list mode: which alpha masks serve their single-key x_b != 0 groups from the column list -------------
+    auto listable = [](const HostGroup& g) { return g.xb != 0 && g.s.front().zb == g.s.back().zb; };
+    std::map<u32, int> n_listable;  // per xa
+    for (auto& g : groups_in) n_listable[g.xa] += listable(g) ? 1 : 0;
+    std::map<std::pair<u32, u32>, u32> listed_id;  // (xb, zb0) -> table id, listed tables first
+    std::map<u32, bool> list_mode;
+    for (auto& kv : n_listable) list_mode[kv.first] = kv.second >= 8;
+    for (int pass = 0; pass < 2; ++pass) {
+        listed_id.clear();
+        for (auto& g : groups_in)
+            if (listable(g) && list_mode[g.xa])
+                listed_id.emplace(std::make_pair(g.xb, g.s.front().zb), (u32)listed_id.size());
+        if (pass == 0)  // drop masks that use only a small part of the list (their padding would dominate)
+            for (auto& kv : n_listable)
+                list_mode[kv.first] = list_mode[kv.first] && 10 * kv.second >= 3 * (int)listed_id.size();
+    }
+    if (listed_id.size() > 1024) {
+        listed_id.clear();
+        for (auto& kv : list_mode) kv.second = false;
+    }
+    // within an alpha mask: dense items first, listed items last (stable)
+    std::vector<HostGroup> groups = groups_in;
+    std::stable_sort(groups.begin(), groups.end(), [&](const HostGroup& a, const HostGroup& b) {
+        if (a.xa != b.xa) return a.xa < b.xa;
+        const int la = list_mode[a.xa] && listable(a), lb = list_mode[b.xa] && listable(b);
+        return la < lb;
+    });
     BS_REQUIRE(Db <= 32767, BS_ERR_ARG, "row plan: column space too large for u16 tables");
     std::vector<u32> xa_list, key_dz, key_s0, s_za;
     std::vector<XaHdr> hdrs;
     std::vector<RowItem> items;
     std::vector<double2> s_w;
-    std::vector<uint2> tkeys;
-    std::map<std::pair<u32, u32>, u32> tkey_id;
+    std::vector<uint2> tkeys(listed_id.size());
+    std::map<std::pair<u32, u32>, u32> tkey_id = listed_id;
+    for (auto& kv : listed_id) tkeys[kv.second] = make_uint2(kv.first.first, kv.first.second);
+    const int n_listed = (int)listed_id.size();
     bool real_w = true;
     int max_keys = 0;
     for (size_t g = 0; g < groups.size(); ++g) {
@@ -86,6 +131,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
             h.item0 = (u32)items.size();
             h.key0 = (u32)key_dz.size();
             h.stage = 0;
+            h.item_split = 0xFFFFFFFFu;
             hdrs.push_back(h);
             xa_list.push_back(hg.xa);
         }
@@ -117,6 +163,10 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
             it.tkey = f->second;
         }
         if (hg.xb != 0) hdrs.back().stage = 1;
+        if (list_mode[hg.xa] && listable(hg) && hdrs.back().item_split == 0xFFFFFFFFu) {
+            hdrs.back().item_split = (u32)items.size();
+            hdrs.back().key_split = it.key0;
+        }
         items.push_back(it);
     }
     if (!hdrs.empty()) {
@@ -124,10 +174,15 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
         hdrs.back().key1 = (u32)key_dz.size();
     }
     key_s0.push_back((u32)s_za.size());
+    for (auto& h : hdrs)
+        if (h.item_split == 0xFFFFFFFFu) {
+            h.item_split = h.item1;
+            h.key_split = h.key1;
+        }
     // "simple" alpha masks: one group with x_b = 0, no beta sign and a single key (pad[0] = 1)
     for (auto& h : hdrs) {
         const RowItem& it = items[h.item0];
-        h.pad[0] = (h.item1 - h.item0 == 1 && !h.stage && it.tkey == kTkeyIdent && it.nkeys == 1) ? 1u : 0u;
+        h.simple = (h.item1 - h.item0 == 1 && !h.stage && it.tkey == kTkeyIdent && it.nkeys == 1) ? 1u : 0u;
     }
     bool any_stage = false;
     for (auto& h : hdrs) {
@@ -143,14 +198,15 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     R->max_keys = max_keys;
     R->any_stage = any_stage;
     // ---- launch geometry ---------------------------------------------------------------------
-    // Shared memory: [mbarrier 16 B][V slots: max_keys * 16 B][row window: win_cols * 16 B].
+    // Shared memory: [mbarrier 16 B][V slots: vcap * 16 B][list V slots: (n_listed + 1) * 16 B][row window].
     const int vcap = std::max(max_keys, 512);
-    const size_t fixed = 16 + (size_t)vcap * 16;
+    const size_t fixed = 16 + (size_t)vcap * 16 + (size_t)(n_listed + 1) * 16;
     const size_t smem_max = 227 * 1024 - 1024;
     i64 win = Db;
     int n_win = 1;
     if (any_stage) {
-        const i64 cap = (i64)((smem_max - fixed) / 16);
+        i64 cap = (i64)((smem_max - fixed) / 16);
+        if (const char* w = getenv("BS_ROW_WIN")) cap = std::max<i64>(8, std::min<i64>(cap, atoll(w)));  // tests
         if (Db > cap) {
             n_win = (int)((Db + cap - 1) / cap);
             win = (((Db + n_win - 1) / n_win) + 7) & ~i64(7);
@@ -193,6 +249,22 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
                                           R->d_ttab.p + k0 * R->tstride);
         BS_COUNT_LAUNCH(1);
     }
+    // column list: compaction of the listed tables over table ids
+    R->n_listed = n_listed;
+    R->l_max = 0;
+    if (n_listed > 0) {
+        DevBuf<int> lcnt;
+        BS_CUDA(lcnt.alloc(R->tstride));
+        const unsigned lb = (unsigned)((R->tstride + 255) / 256);
+        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, 0, nullptr, lcnt.p);
+        std::vector<int> hl(R->tstride);
+        BS_CUDA(cudaMemcpyAsync(hl.data(), lcnt.p, R->tstride * 4, cudaMemcpyDeviceToHost, st));
+        BS_CUDA(cudaStreamSynchronize(st));
+        for (int v : hl) R->l_max = std::max(R->l_max, v);
+        BS_CUDA(R->d_ltab.alloc((size_t)std::max(1, R->l_max) * R->tstride));
+        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, R->l_max, R->d_ltab.p, lcnt.p);
+        BS_COUNT_LAUNCH(2);
+    }
     // per-row valid alpha masks
     DevBuf<int> cnt;
     BS_CUDA(cnt.alloc(Da));
@@ -229,5 +301,8 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const 
     d.win_cols = R->win_cols;
     d.n_win = R->n_win;
     d.chunk_cols = R->chunk_cols;
+    d.ltab = R->d_ltab.p;
+    d.l_max = R->l_max;
+    d.n_listed = n_listed;
     return BS_OK;
 }

@@ -21,7 +21,9 @@ struct __align__(16) XaHdr {
     u32 item0, item1;  // items (groups) under this alpha mask
     u32 key0, key1;    // their keys, contiguous: V slot of key k is k - key0
     u32 stage;         // 1: some item has xb != 0 -> the source row is staged in shared memory
-    u32 pad[3];
+    u32 simple;        // 1: one group, x_b = 0, no beta sign, one key: a plain row axpy
+    u32 item_split;    // items [item_split, item1) are single-key x_b != 0 groups served by the column LIST
+    u32 key_split;     // first key of those items (they own one key each, in item order)
 };
 struct __align__(16) RowItem {
     u32 tkey;   // column table id or kTkeyIdent
@@ -49,6 +51,10 @@ struct RowPlanDev {
     int win_cols;               // columns of a source row staged at once (>= Db: whole row)
     int n_win;                  // number of windows
     int chunk_cols;             // target columns per thread block
+    // Column list (compaction of the listed column tables over table ids): entry j of slot s is
+    // source column | sign << 15 | table id << 16; padded with (0, 0, n_listed) whose V slot is always 0.
+    const u32* ltab;            // [l_max][tstride]
+    int l_max, n_listed;
 };
 
 struct bs_rowplan {
@@ -62,6 +68,8 @@ struct bs_rowplan {
     DevBuf<u32> d_key_dz, d_key_s0, d_s_za;
     DevBuf<double2> d_s_w;
     DevBuf<unsigned short> d_ttab;
+    DevBuf<u32> d_ltab;
+    int l_max = 0, n_listed = 0;
     DevBuf<i64> d_row_off;
     DevBuf<uint4> d_row_ent;
     i64 tstride = 0;
