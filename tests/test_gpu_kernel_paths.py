@@ -1,0 +1,83 @@
+"""GPU parity of every apply-kernel path against the oracle on the same operators.
+
+The library picks its path per (operator, sector): v2 row kernel (default), windowed source rows when a
+row exceeds shared memory, beta-only groups on the transposed problem or in-row, and the v1 kernel as
+fallback.  The environment switches below (read when a plan is built) force each path on sizes the
+definition-mode oracle finishes in seconds; each runs in a fresh interpreter because plans are cached.
+"""
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+SCRIPT = r"""
+import sys, os
+sys.path.insert(0, sys.argv[1]); sys.path.insert(0, os.path.join(sys.argv[1], 'tests'))
+import numpy as np, torch
+import synth_inputs as si
+from common import oracle_operator, raw_terms, rel_l2
+from oracle import oracle as orc
+from paper_2606_28952_b200 import bs, jw_terms as jw
+want_kernel = sys.argv[2]
+rng = np.random.default_rng(3)
+cases = []
+for name in ('q12', 'q24'):
+    cfg = si.CONFIGS[name]
+    cases.append((name, oracle_operator(name), raw_terms(name), cfg.n_orb, cfg.n_alpha, cfg.n_beta))
+ref8 = orc.hubbard_h(8, 1.0, 4.0)
+cases.append(('hub8', ref8, jw.hubbard_raw_terms(8, 1.0, 4.0), 8, 4, 3))
+h, g = si.integrals(7, 77)
+cases.append(('mol7', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 7, 2, 5))
+# generic complex operator (multi-key, POPC signs, complex weights)
+M = 400
+x = rng.integers(0, 1 << 12, M, dtype=np.uint64); x[:60] = 0; x[60:150] = 0b000011; x[150:260] = 0b000101000011
+x[260:300] = 0b011000000000
+z = rng.integers(0, 1 << 12, M, dtype=np.uint64)
+c = rng.standard_normal(M) + 1j * rng.standard_normal(M)
+for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2)]:
+    op = bs.bs_group_xmask(*raw, 2 * n, 1e-12 if ref is not None else 0.0)
+    if ref is None:
+        xg, offs, zz, cc, _ = op.export()
+        ref = orc.PauliOp(np.repeat(xg, np.diff(offs)), zz, cc)
+    sec, osec = bs.bs_sector_build(n, na, nb), orc.Sector(n, na, nb)
+    desc = bs.bs_plan_describe(op, sec)
+    assert want_kernel in desc, (want_kernel, desc)
+    psi = si.random_state(osec.dim, 5)
+    want = osec.apply_grouped(ref, psi) if osec.dim > 100000 else osec.apply(ref, psi)
+    d_in = torch.from_numpy(psi).cuda(); d_out = torch.full_like(d_in, float('nan'))
+    bs.bs_apply(op, sec, d_in, d_out)
+    err = rel_l2(d_out.cpu().numpy(), want)
+    e = bs.bs_expect(op, sec, d_in)
+    de = abs(e - orc.vdot(psi, want))
+    # row slab + fused epilogue on the same path
+    lo, hi = osec.dim_alpha // 3, (2 * osec.dim_alpha) // 3 + 1
+    d_slab = torch.zeros_like(d_in); bs.bs_apply_rows(op, sec, d_in, d_slab, lo, hi)
+    slab = d_slab.cpu().numpy(); Db = osec.dim_beta
+    err_s = rel_l2(slab[lo * Db:hi * Db], want[lo * Db:hi * Db])
+    assert np.all(slab[:lo * Db] == 0) and np.all(slab[hi * Db:] == 0)
+    acc0 = si.random_state(osec.dim, 6); d_acc = torch.from_numpy(acc0).cuda(); d_o2 = torch.zeros_like(d_in)
+    bs.bs_apply_axpby(op, sec, d_in, d_o2, 0.5 - 2j, 1.5j, d_acc)
+    w2 = (0.5 - 2j) * want + 1.5j * psi
+    err_a = max(rel_l2(d_o2.cpu().numpy(), w2), rel_l2(d_acc.cpu().numpy(), acc0 + w2))
+    print(name, desc.split(' ')[0], f"{err:.2e} {de:.2e} {err_s:.2e} {err_a:.2e}")
+    assert err <= 1e-12 and de <= 1e-10 and err_s <= 1e-12 and err_a <= 1e-12, (name, err, de, err_s, err_a)
+print('PATH OK')
+"""
+
+
+@pytest.mark.parametrize("env,kernel", [
+    ({}, "rows_v2"),
+    ({"BS_KERNEL": "v1"}, "sector_v1"),
+    ({"BS_KERNEL": "v2inrow"}, "rows_v2"),
+    ({"BS_ROW_WIN": "24"}, "n_win="),
+    ({"BS_ROW_WIN": "24", "BS_KERNEL": "v2inrow"}, "rows_v2"),
+])
+def test_kernel_path(env, kernel):
+    e = dict(os.environ)
+    e.update(env)
+    r = subprocess.run([sys.executable, "-c", SCRIPT, ROOT, kernel], env=e, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "PATH OK" in r.stdout, r.stdout[-3000:] + r.stderr[-3000:]
