@@ -72,9 +72,9 @@ print('PATH OK')
 @pytest.mark.parametrize("env,kernel", [
     ({}, "rows_v2"),
     ({"BS_KERNEL": "v1"}, "sector_v1"),
-    ({"BS_KERNEL": "v2inrow"}, "rows_v2"),
+    ({"BS_KERNEL": "v2inrow"}, "kernel="),      # q24's beta-only groups do not fit in-row: falls back to v1 there
     ({"BS_ROW_WIN": "24"}, "n_win="),
-    ({"BS_ROW_WIN": "24", "BS_KERNEL": "v2inrow"}, "rows_v2"),
+    ({"BS_ROW_WIN": "24", "BS_KERNEL": "v2inrow"}, "kernel="),
 ])
 def test_kernel_path(env, kernel):
     e = dict(os.environ)
