@@ -131,7 +131,7 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
     b.record()
     torch.cuda.synchronize()
     first_ms = a.elapsed_time(b)
-    reps = 0 if first_ms > 20000 else (3 if first_ms > 500 else 10)
+    reps = 0 if first_ms > 30000 else (2 if first_ms > 2000 else (3 if first_ms > 500 else 10))
     times = []
     for _ in range(reps):
         if flush:
@@ -144,6 +144,7 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
         times.append(a.elapsed_time(b))
     apply_ms = _median(times) if times else first_ms
     ent = {"n_qubits": cfg.n_qubits, "dim": cfg.dim, "groups": op.n_groups, "strings": op.n_terms,
+           "plan": bs.bs_plan_describe(op, sec),
            "raw_terms": m_raw, "raw_terms_s": round(t_raw, 3), "setup_s": round(t_setup, 3),
            "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
            "l2_flush_between_reps": bool(flush)}
@@ -294,7 +295,7 @@ def run_ours(args):
     applies_per_step = TAYLOR_ORDER + 1
     if rank == 0:
         value = world * applies_per_step * args.steps / (total_ms * 1e-3)
-        # dominant kernel: k_apply_sector (Taylor launches). Algorithmic bytes per Taylor step:
+        # dominant kernel: k_rows (Taylor launches). Algorithmic bytes per Taylor step:
         # k=1: 32 D; k=2..order-1: 64 D (in, out, acc r+w); k=order: 48 D; + tables each launch.
         bytes_taylor = (32 + 64 * (TAYLOR_ORDER - 2) + 48) * D + TAYLOR_ORDER * tb
         launch_ms = taylor_ms / (args.steps * TAYLOR_ORDER)
@@ -309,13 +310,14 @@ def run_ours(args):
                        "step": f"1 Taylor-{TAYLOR_ORDER} step (dt={DT}, shifted) + 1 bs_expect = "
                                f"{applies_per_step} H applies",
                        "l2": "3 vectors x 188.5 MB > 126 MB L2, no flush needed",
-                       "parallelism": f"{world} independent state vector(s), one per GPU"},
+                       "parallelism": f"{world} independent state vector(s), one per GPU",
+                       "plan": bs.bs_plan_describe(op, sec)},
             "setup_ms": setup_ms, "taylor_ms_per_step": taylor_ms / args.steps,
             "expect_ms_per_call": expect_ms / args.steps, "energy": energy.real, "norm_drift": norm_drift,
             "gpu_launches": int(launches), "clocks": clocks,
             "e2e": {"value": world * applies_per_step * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 16 * D, "d2h_bytes_per_step": 16 * D + 16, "steps": e2e_steps},
-            "roofline": {"bound": "hbm", "kernel": "k_apply_sector (fused apply+axpy launches of bs_taylor_step)",
+            "roofline": {"bound": "hbm", "kernel": "k_rows<MODE_FINAL> (fused apply+axpy launches of bs_taylor_step)",
                          "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
                          "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
                          "launch_ms": launch_ms, "traffic": TRAFFIC_NCU.get(name)},
@@ -387,11 +389,11 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="q28_hubbard", choices=si.CONFIG_ORDER)
-    ap.add_argument("--per-config", default="q12,q24,q28_hubbard,q32",
+    ap.add_argument("--per-config", default="q12,q24,q28_hubbard,q32,q56",
                     help="comma list of configs to time with plain bs_apply (N=1 only), or 'none'")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
