@@ -169,10 +169,11 @@ __device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT
                                           const double2* __restrict__ srow, u32 w0, u32 wn, u32 tpos,
                                           double2 (&acc)[CPT]) {
     using V = VT<REALW>;
-    const u32* __restrict__ L = P.ltab + tpos;
+    const u32* __restrict__ p = P.ltab + tpos;
+    const u32 stride = (u32)P.tstride;
+    const int l_max = P.l_max;
     u32 en[CPT], nx[CPT];
-    auto load = [&](int j, u32 (&e)[CPT]) {
-        const u32* p = L + (i64)j * P.tstride;
+    auto load = [&](u32 (&e)[CPT]) {
         if (CPT == 4) {
             const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
             e[0] = v.x;
@@ -183,12 +184,14 @@ __device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT
 #pragma unroll
             for (int c = 0; c < CPT; ++c) e[c] = __ldg(p + c);
         }
+        p += stride;
     };
-    load(0, nx);
-    for (int j = 0; j < P.l_max; ++j) {
+    load(nx);
+#pragma unroll 1
+    for (int j = 0; j < l_max; ++j) {
 #pragma unroll
         for (int c = 0; c < CPT; ++c) en[c] = nx[c];
-        if (j + 1 < P.l_max) load(j + 1, nx);
+        if (j + 1 < l_max) load(nx);
 #pragma unroll
         for (int c = 0; c < CPT; ++c) {
             const u32 src = en[c] & 0x7FFFu;
