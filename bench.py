@@ -250,12 +250,15 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing ------------------------------------------------------------------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()            # nvidia-smi needs ~0.5 s to deliver its first sample: start before warm-up
     for _ in range(args.warmup):
         step()
-    sampler = ClockSampler(local)
+    t_w = time.perf_counter()
+    while time.perf_counter() - t_w < 0.6:      # keep the GPU under load until the sampler is live
+        step()
     barrier()
-    if rank == 0:
-        sampler.start()
     n0 = bs.bs_launch_count()
     marks = [ev() for _ in range(2 * args.steps + 1)]
     marks[0].record()
@@ -338,7 +341,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {}
+TRAFFIC_NCU = {"q28_hubbard": 1.0356e9}   # profiles/r01_v2_q28_k_rows_full.md, fused apply+axpy launch
 
 
 def run_reference(args):
