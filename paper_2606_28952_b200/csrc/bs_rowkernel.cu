@@ -164,15 +164,17 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
 
 // Column-list pass of a staged entry: every single-key x_b != 0 group under the alpha mask, compacted per
 // column (no invalid lanes, no branches): entry = source column | sign << 15 | table id << 16, V from sVx[id].
-template <bool REALW, int CPT, bool WINDOWED>
+// Padding entries point at column Db (a zero amplitude kept behind the staged row) with id n_listed (V = 0).
+// UNIF: every listed group has the same row-independent weight `vu` (lattice hopping terms): no V lookup.
+template <bool REALW, int CPT, bool WINDOWED, bool UNIF>
 __device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT<REALW>::type* __restrict__ sVx,
-                                          const double2* __restrict__ srow, u32 w0, u32 wn, u32 tpos,
-                                          double2 (&acc)[CPT]) {
+                                          typename VT<REALW>::type vu, const double2* __restrict__ srow, u32 w0, u32 wn,
+                                          u32 tpos, double2 (&acc)[CPT]) {
     using V = VT<REALW>;
     const u32* __restrict__ p = P.ltab + tpos;
     const u32 stride = (u32)P.tstride;
     const int l_max = P.l_max;
-    u32 en[CPT], nx[CPT];
+    u32 en[CPT], n1[CPT];
     auto load = [&](u32 (&e)[CPT]) {
         if (CPT == 4) {
             const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
@@ -186,17 +188,17 @@ __device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT
         }
         p += stride;
     };
-    load(nx);
+    load(n1);
 #pragma unroll 1
     for (int j = 0; j < l_max; ++j) {
 #pragma unroll
-        for (int c = 0; c < CPT; ++c) en[c] = nx[c];
-        if (j + 1 < l_max) load(nx);
+        for (int c = 0; c < CPT; ++c) en[c] = n1[c];
+        if (j + 1 < l_max) load(n1);
 #pragma unroll
         for (int c = 0; c < CPT; ++c) {
             const u32 src = en[c] & 0x7FFFu;
             if (WINDOWED && (src - w0) >= wn) continue;
-            V::fma(acc[c], sVx[en[c] >> 16], (en[c] >> 15) & 1u, srow[src - w0]);
+            V::fma(acc[c], UNIF ? vu : sVx[en[c] >> 16], (en[c] >> 15) & 1u, srow[src - w0]);
         }
     }
 }
@@ -234,6 +236,7 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
     if (tid == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        srow[P.win_cols] = make_double2(0.0, 0.0);  // target of the column list's padding entries
     }
     u32 phase = 0;
     const uint4* __restrict__ items4 = reinterpret_cast<const uint4*>(P.items);
@@ -257,7 +260,8 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
         const double2* __restrict__ srow_g = psi + (i64)first.y * Db;  // staged batches have one entry
         const uint4 hs = __ldg(reinterpret_cast<const uint4*>(P.xa_hdr + first.x) + 1);  // stage,simple,item_split,key_split
         const u32 item_end = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + first.x) + 1);
-        const bool listed = stage && hs.z < item_end;
+        const bool listed = (stage & 1u) && hs.z < item_end;
+        const bool unif = (hs.x & 2u) != 0;  // all listed groups share one row-independent weight
         __syncthreads();  // everyone is done with the previous batch's V slots and staged row
         if (listed) {
             for (int k = tid; k <= P.n_listed; k += nt) sVx[k] = V::zero();
@@ -321,12 +325,15 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                     if (h4.x < hs.z)
                         process_entry<REALW, CPT, true, false>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, 0u, wn,
                                                                tpos, col, tb, acc);
-                    if (listed) list_pass<REALW, CPT, false>(P, sVx, srow, 0u, wn, tpos, acc);
+                    if (listed) {
+                        if (unif) list_pass<REALW, CPT, false, true>(P, sVx, vbase[hs.w - h4.z], srow, 0u, wn, tpos, acc);
+                        else list_pass<REALW, CPT, false, false>(P, sVx, V::zero(), srow, 0u, wn, tpos, acc);
+                    }
                 } else {
                     if (h4.x < hs.z)
                         process_entry<REALW, CPT, true, true>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, w0, wn,
                                                               tpos, col, tb, acc);
-                    if (listed) list_pass<REALW, CPT, true>(P, sVx, srow, w0, wn, tpos, acc);
+                    if (listed) list_pass<REALW, CPT, true, false>(P, sVx, V::zero(), srow, w0, wn, tpos, acc);
                 }
             }
         }

@@ -32,7 +32,7 @@ __global__ void k_fill_ttab(SpinTab B, const uint2* __restrict__ keys, i64 tstri
 }
 
 // l_max == 0: count the valid listed tables of every slot; else write the padded list
-__global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, int n_listed, int l_max,
+__global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, int n_listed, int l_max, u32 pad_src,
                              u32* __restrict__ L, int* __restrict__ cnt) {
     const i64 slot = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (slot >= tstride) return;
@@ -44,7 +44,7 @@ __global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, 
         ++j;
     }
     if (!l_max) cnt[slot] = j;
-    else for (; j < l_max; ++j) L[(i64)j * tstride + slot] = (u32)n_listed << 16;
+    else for (; j < l_max; ++j) L[(i64)j * tstride + slot] = pad_src | ((u32)n_listed << 16);
 }
 
 __global__ void k_row_count2(SpinTab A, const u32* __restrict__ xa, int n_xa, int* __restrict__ cnt) {
@@ -70,7 +70,7 @@ __global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* 
         u32 m = __ldg(xa + i);
         if (2 * __popc(ta & m) == __popc(m)) {
             const u32 nk = hdr[i].key1 - hdr[i].key0;
-            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | (hdr[i].stage << 31) | (hdr[i].simple << 30));
+            ent[o++] = make_uint4((u32)i, spin_rank(A, ta ^ m), koff, nk | ((hdr[i].stage & 1u) << 31) | (hdr[i].simple << 30));
             koff += nk;
         }
     }
@@ -179,6 +179,17 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
             h.item_split = h.item1;
             h.key_split = h.key1;
         }
+    // stage bit 1: every listed group has a single string with z_a = 0 and the same weight
+    for (auto& h : hdrs) {
+        if (h.item_split >= h.item1) continue;
+        bool unif = true;
+        const u32 s_first = key_s0[items[h.item_split].key0];
+        for (u32 i = h.item_split; i < h.item1 && unif; ++i) {
+            const u32 k = items[i].key0, sa = key_s0[k], sb = key_s0[k + 1];
+            unif = (sb - sa == 1) && s_za[sa] == 0 && s_w[sa].x == s_w[s_first].x && s_w[sa].y == s_w[s_first].y;
+        }
+        if (unif) h.stage |= 2u;
+    }
     // "simple" alpha masks: one group with x_b = 0, no beta sign and a single key (pad[0] = 1)
     for (auto& h : hdrs) {
         const RowItem& it = items[h.item0];
@@ -205,7 +216,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     i64 win = Db;
     int n_win = 1;
     if (any_stage) {
-        i64 cap = (i64)((smem_max - fixed) / 16);
+        i64 cap = (i64)((smem_max - fixed) / 16) - 1;
         if (const char* w = getenv("BS_ROW_WIN")) cap = std::max<i64>(8, std::min<i64>(cap, atoll(w)));  // tests
         if (Db > cap) {
             n_win = (int)((Db + cap - 1) / cap);
@@ -214,12 +225,13 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     } else win = 0;
     R->win_cols = (int)win;
     R->n_win = n_win;
-    R->smem = fixed + (size_t)win * 16;
+    R->smem = fixed + (size_t)win * 16 + 16;  // + the zero amplitude behind the row (list padding)
     // threads / columns per thread: small rows -> several blocks per SM; big rows -> 1024 threads
     int threads, cpt;
     if (R->smem > 110 * 1024) threads = 1024;
     else if (R->smem > 56 * 1024 || Db >= 2048) threads = 512;
     else threads = 256;
+    if (const char* t = getenv("BS_ROW_THREADS")) threads = std::max(64, std::min(1024, atoi(t)) & ~31);  // tuning / tests
     const i64 per_block_max = (i64)threads * 4;
     int n_chunks = (int)((Db + per_block_max - 1) / per_block_max);
     i64 chunk = ((Db + n_chunks - 1) / n_chunks + 31) & ~i64(31);
@@ -256,13 +268,13 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
         DevBuf<int> lcnt;
         BS_CUDA(lcnt.alloc(R->tstride));
         const unsigned lb = (unsigned)((R->tstride + 255) / 256);
-        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, 0, nullptr, lcnt.p);
+        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, 0, 0u, nullptr, lcnt.p);
         std::vector<int> hl(R->tstride);
         BS_CUDA(cudaMemcpyAsync(hl.data(), lcnt.p, R->tstride * 4, cudaMemcpyDeviceToHost, st));
         BS_CUDA(cudaStreamSynchronize(st));
         for (int v : hl) R->l_max = std::max(R->l_max, v);
         BS_CUDA(R->d_ltab.alloc((size_t)std::max(1, R->l_max) * R->tstride));
-        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, R->l_max, R->d_ltab.p, lcnt.p);
+        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, R->l_max, (u32)Db, R->d_ltab.p, lcnt.p);
         BS_COUNT_LAUNCH(2);
     }
     // per-row valid alpha masks
