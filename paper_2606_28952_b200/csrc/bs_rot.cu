@@ -31,12 +31,21 @@ __device__ __forceinline__ double2 phase_sum(const u64* __restrict__ z, const do
     return make_double2(fr, fi);
 }
 
-__device__ __forceinline__ void rotate_pair(double2* __restrict__ psi, i64 it, i64 iu, double2 F, double theta) {
-    const double r = hypot(F.x, F.y);
-    if (r == 0.0) return;
+// sc1 = (sin theta, cos theta) precomputed on the host for the common case |F| = 1 (fermionic excitation
+// generators: |f| is 0 or 1); other moduli take the sincos path.
+__device__ __forceinline__ void rotate_pair(double2* __restrict__ psi, i64 it, i64 iu, double2 F, double theta,
+                                            double2 sc1) {
+    const double r2 = F.x * F.x + F.y * F.y;
+    if (r2 == 0.0) return;
     double sn, cs;
-    sincos(theta * r, &sn, &cs);
-    sn /= r;
+    if (r2 == 1.0) {
+        sn = sc1.x;
+        cs = sc1.y;
+    } else {
+        const double r = hypot(F.x, F.y);
+        sincos(theta * r, &sn, &cs);
+        sn /= r;
+    }
     const double2 a = psi[it], b = psi[iu];
     // psi'[t] = cs a + sn F b ; psi'[u] = cs b - sn conj(F) a
     psi[it] = make_double2(cs * a.x + sn * (F.x * b.x - F.y * b.y), cs * a.y + sn * (F.x * b.y + F.y * b.x));
@@ -45,18 +54,21 @@ __device__ __forceinline__ void rotate_pair(double2* __restrict__ psi, i64 it, i
 
 __global__ void __launch_bounds__(256)
 k_rot_sector(SpinTab A, SpinTab B, int n_orb, u64 x, const u64* __restrict__ z, const double2* __restrict__ w, int k0,
-             int k1, double theta, double2* __restrict__ psi) {
-    const i64 i = blockIdx.x * (i64)blockDim.x + threadIdx.x;
-    if (i >= A.D * B.D) return;
-    const u32 row = (u32)(i / B.D), col = (u32)(i - (i64)row * B.D);
-    const u32 ta = A.str[row], tb = B.str[col];
+             int k1, double theta, double2 sc1, double2* __restrict__ psi) {
+    // grid: x = column blocks, y = alpha rows (no 64-bit division); the alpha test is uniform per block
+    const u32 row = blockIdx.y, col = blockIdx.x * blockDim.x + threadIdx.x;
     const u32 xa = (u32)(x & ((u64(1) << n_orb) - 1)), xb = (u32)(x >> n_orb);
-    const u64 t = (u64)ta | ((u64)tb << n_orb);
-    const bool valid = (2 * __popc(ta & xa) == __popc(xa)) && (2 * __popc(tb & xb) == __popc(xb));
-    if (!valid) return;  // partner outside the sector: F(t) = 0 there (checked once by k_rot_leak_check)
-    const i64 iu = (i64)spin_rank(A, ta ^ xa) * B.D + spin_rank(B, tb ^ xb);
-    if (iu < i) return;  // the pair belongs to its smaller index (x != 0, so iu != i)
-    rotate_pair(psi, i, iu, phase_sum(z, w, k0, k1, t), theta);
+    const u32 ta = A.str[row];
+    if (2 * __popc(ta & xa) != __popc(xa)) return;  // partner outside the sector: F = 0 there (leak check)
+    if (col >= B.D) return;
+    const u32 tb = B.str[col];
+    if (2 * __popc(tb & xb) != __popc(xb)) return;
+    const u32 urow = xa ? spin_rank(A, ta ^ xa) : row;
+    if (urow < row) return;  // the pair belongs to its smaller index (x != 0, so iu != i)
+    const u32 ucol = xb ? spin_rank(B, tb ^ xb) : col;
+    if (urow == row && ucol < col) return;
+    const i64 i = (i64)row * B.D + col, iu = (i64)urow * B.D + ucol;
+    rotate_pair(psi, i, iu, phase_sum(z, w, k0, k1, (u64)ta | ((u64)tb << n_orb)), theta, sc1);
 }
 
 // One-off validation of a generator list against a sector: for every generator (blockIdx.y) and
@@ -79,12 +91,12 @@ k_rot_leak_check(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, co
 
 __global__ void __launch_bounds__(256)
 k_rot_full(i64 D, u64 x, const u64* __restrict__ z, const double2* __restrict__ w, int k0, int k1, double theta,
-           double2* __restrict__ psi) {
+           double2 sc1, double2* __restrict__ psi) {
     const i64 i = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (i >= D) return;
     const i64 iu = i ^ (i64)x;
     if (iu < i) return;
-    rotate_pair(psi, i, iu, phase_sum(z, w, k0, k1, (u64)i), theta);
+    rotate_pair(psi, i, iu, phase_sum(z, w, k0, k1, (u64)i), theta, sc1);
 }
 
 }  // namespace
@@ -136,13 +148,16 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
         BS_REQUIRE(!leak, BS_ERR_LEAVES_SECTOR, "a generator maps the sector outside itself");
         gen->validated_sectors.push_back(s->id);
     }
+    const dim3 sgrid((unsigned)((s->Db + 255) / 256), (unsigned)std::min<i64>(s->Da, 65535));
+    BS_REQUIRE(s->full || s->Da <= 65535, BS_ERR_ARG, "bs_apply_pauli_rotations: more than 65535 alpha strings");
     for (i64 j = 0; j < n_rot; ++j) {
         const int k0 = (int)gen->h_offs[j], k1 = (int)gen->h_offs[j + 1];
+        const double2 sc1 = make_double2(sin(thetas[j]), cos(thetas[j]));
         if (s->full)
-            k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], psi);
+            k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
         else
-            k_rot_sector<<<nb, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1,
-                                             thetas[j], psi);
+            k_rot_sector<<<sgrid, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1,
+                                                thetas[j], sc1, psi);
     }
     BS_COUNT_LAUNCH(n_rot);
     BS_CUDA(cudaGetLastError());
