@@ -99,6 +99,17 @@ def build_operator_terms(name: str):
     return jw.molecular_raw_terms(h, g)
 
 
+def build_operator(name: str, bs):
+    """a1 + a2 on the device, fed by the device-side JW construction (bs_jw_*): returns (op, raw term count)."""
+    cfg = si.CONFIGS[name]
+    if cfg.kind == "hubbard":
+        L = cfg.n_orb
+        return bs.bs_jw_hubbard(L, cfg.hubbard_t, cfg.hubbard_u), (L - 1) * 16 + L * 16
+    h, g = si.integrals(cfg.n_orb, cfg.seed_ints)
+    n = cfg.n_orb
+    return bs.bs_jw_molecular(h, g), 8 * n * n + 64 * n ** 4
+
+
 def table_bytes(op) -> int:
     """Group-table bytes of the a2 layout: xg u64[G] + offs i64[G+1] + z u64[M] + w c128[M]."""
     return 8 * op.n_groups + 8 * (op.n_groups + 1) + 24 * op.n_terms
@@ -112,15 +123,10 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
     """Plain bs_apply / bs_expect timings of one BASELINE.json config (CUDA events, median)."""
     cfg = si.CONFIGS[name]
     t0 = time.perf_counter()
-    raw = build_operator_terms(name)
-    t_raw = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    op = bs.bs_group_xmask(*raw, cfg.n_qubits, 1e-12)
+    op, m_raw = build_operator(name, bs)
     sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t0
-    m_raw = len(raw[0])
-    del raw
     psi = torch.from_numpy(si.random_state(cfg.dim, cfg.seed_psi)).cuda()
     out = torch.empty_like(psi)
     flush = 16 * cfg.dim * 2 < 126e6                      # both vectors would sit in the 126 MB L2
@@ -145,7 +151,7 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
     apply_ms = _median(times) if times else first_ms
     ent = {"n_qubits": cfg.n_qubits, "dim": cfg.dim, "groups": op.n_groups, "strings": op.n_terms,
            "plan": bs.bs_plan_describe(op, sec),
-           "raw_terms": m_raw, "raw_terms_s": round(t_raw, 3), "setup_s": round(t_setup, 3),
+           "raw_terms": m_raw, "setup_s": round(t_setup, 3),
            "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
            "l2_flush_between_reps": bool(flush)}
     bytes_alg = 32 * cfg.dim + table_bytes(op)
@@ -226,12 +232,10 @@ def run_ours(args):
 
     # ---- setup (a1-a3), outside the timed region ------------------------------------------------
     t0 = time.perf_counter()
-    raw = build_operator_terms(name)
-    op = bs.bs_group_xmask(*raw, cfg.n_qubits, 1e-12)
+    op, _ = build_operator(name, bs)
     sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
     torch.cuda.synchronize()
     setup_ms = (time.perf_counter() - t0) * 1e3
-    del raw
     psi_h = torch.from_numpy(si.random_state(D, cfg.seed_psi + rank)).pin_memory()   # one state per rank
     out_h = torch.empty_like(psi_h).pin_memory()
     psi = psi_h.cuda()

@@ -73,6 +73,15 @@ int bs_op_info(bs_op_t op, int64_t* n_groups, int64_t* n_terms, int* n_qubits);
 int bs_op_export(bs_op_t op, uint64_t* xg, int64_t* offs, uint64_t* z, double* c_reim, double* w_reim);
 int bs_op_destroy(bs_op_t op);
 
+/* ---- device-side Jordan-Wigner construction (Alg. 1) feeding a1/a2 directly: the raw 4/16-term
+ * expansions are generated and reduced on the device.  h [host] double[n_orb^2] symmetric one-body integrals,
+ * g [host] double[n_orb^4] two-body integrals in chemist notation (pq|rs), row-major g[p][q][r][s];
+ * H = sum h_pq a+_{ps} a_{qs} + 1/2 sum (pq|rs) a+_{ps} a+_{rt} a_{st} a_{qs}, blocked spin ordering (2 n_orb qubits).
+ * bs_jw_hubbard: open chain, H = -t sum (a+_{is} a_{i+1,s} + h.c.) + U sum n_{i,alpha} n_{i,beta}.
+ * The resulting operator is a BS_MODE_CANONICAL operator (same tables as bs_group_xmask on the raw list). */
+int bs_jw_molecular(int n_orb, const double* h, const double* g, double eps_drop, void* cuda_stream, bs_op_t* out);
+int bs_jw_hubbard(int n_sites, double t, double U, double eps_drop, void* cuda_stream, bs_op_t* out);
+
 /* ---- a3: sector tables.  n_alpha = n_beta = -1: full 2^n space and
  * n_orb then means n_qubits.  Sector mode needs n_orb <= 32, 0 <= n_alpha, n_beta <= n_orb. */
 int bs_sector_build(int n_orb, int n_alpha, int n_beta, void* cuda_stream, bs_sector_t* out);

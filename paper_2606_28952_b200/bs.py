@@ -25,7 +25,7 @@ SYMBOLS = [
     "bs_group_xmask", "bs_op_info", "bs_op_export", "bs_op_destroy",
     "bs_sector_build", "bs_sector_info", "bs_sector_export", "bs_sector_rank", "bs_sector_destroy",
     "bs_apply", "bs_apply_rows", "bs_apply_axpby", "bs_expect", "bs_vdot",
-    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_launch_count", "bs_last_error", "bs_version",
+    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
 ]
 
 
@@ -58,6 +58,8 @@ def _load():
     L.bs_vdot.argtypes = [vp, vp, vp, C.POINTER(dbl), vp]
     L.bs_apply_pauli_rotations.argtypes = [vp, vp, vp, i64, vp, vp]
     L.bs_taylor_step.argtypes = [vp, vp, vp, vp, dbl, C.c_int, dbl, vp]
+    L.bs_jw_molecular.argtypes = [C.c_int, vp, vp, dbl, vp, C.POINTER(vp)]
+    L.bs_jw_hubbard.argtypes = [C.c_int, dbl, dbl, dbl, vp, C.POINTER(vp)]
     L.bs_plan_describe.argtypes = [vp, vp, C.c_char_p, i64, vp]
     L.bs_launch_count.restype = i64
     L.bs_last_error.restype = C.c_char_p
@@ -250,3 +252,21 @@ def bs_plan_describe(op: Op, sector: Sector, stream=None) -> str:
     buf = C.create_string_buffer(1024)
     _check(_lib.bs_plan_describe(op._h, sector._h, buf, 1024, _stream(stream)))
     return buf.value.decode()
+
+
+def bs_jw_molecular(h, g, eps_drop: float = 1e-12, stream=None) -> Op:
+    """Device-side JW construction + canonical reduction of a molecular Hamiltonian (chemist-notation g)."""
+    h = np.ascontiguousarray(h, np.float64)
+    g = np.ascontiguousarray(g, np.float64)
+    n = h.shape[0]
+    if h.shape != (n, n) or g.shape != (n, n, n, n):
+        raise ValueError("h must be [n, n] and g [n, n, n, n]")
+    out = C.c_void_p()
+    _check(_lib.bs_jw_molecular(n, _np_ptr(h), _np_ptr(g), eps_drop, _stream(stream), C.byref(out)))
+    return Op(out)
+
+
+def bs_jw_hubbard(n_sites: int, t: float, U: float, eps_drop: float = 1e-12, stream=None) -> Op:
+    out = C.c_void_p()
+    _check(_lib.bs_jw_hubbard(n_sites, t, U, eps_drop, _stream(stream), C.byref(out)))
+    return Op(out)

@@ -124,8 +124,11 @@ int finish_op(bs_op* op, const u64* d_x_per_string, const double2* d_c, cudaStre
     return BS_OK;
 }
 
-int group_canonical(bs_op* op, const u64* hx, const u64* hz, const double* hc, i64 M0, double eps,
-                    cudaStream_t st) {
+}  // namespace
+
+// canonical reduction + grouping of raw terms that already live on the device (x0, z0, c0 [M0])
+int bs_group_canonical_dev(bs_op* op, const u64* x0p, const u64* z0p, const double2* c0p, i64 M0, double eps,
+                           cudaStream_t st) {
     const int nq = op->n_qubits;
     if (M0 == 0) {
         op->G = 0;
@@ -137,19 +140,20 @@ int group_canonical(bs_op* op, const u64* hx, const u64* hz, const double* hc, i
         BS_CUDA(cudaMemsetAsync(op->d_offs.p, 0, 8, st));
         return finish_op(op, nullptr, nullptr, st);
     }
-    DevBuf<u64> x0, z0, ka, kb;
-    DevBuf<double2> c0;
+    struct View {
+        const u64* p;
+    };
+    struct ViewC {
+        const double2* p;
+    };
+    const View x0{x0p}, z0{z0p};
+    const ViewC c0{c0p};
+    DevBuf<u64> ka, kb;
     DevBuf<u32> ia, ib;
-    BS_CUDA(x0.alloc(M0));
-    BS_CUDA(z0.alloc(M0));
-    BS_CUDA(c0.alloc(M0));
     BS_CUDA(ka.alloc(M0));
     BS_CUDA(kb.alloc(M0));
     BS_CUDA(ia.alloc(M0));
     BS_CUDA(ib.alloc(M0));
-    BS_CUDA(cudaMemcpyAsync(x0.p, hx, M0 * 8, cudaMemcpyHostToDevice, st));
-    BS_CUDA(cudaMemcpyAsync(z0.p, hz, M0 * 8, cudaMemcpyHostToDevice, st));
-    BS_CUDA(cudaMemcpyAsync(c0.p, hc, M0 * 16, cudaMemcpyHostToDevice, st));
 
     // 1. stable sort by (x, z): LSD over the two 64-bit words
     size_t tmp_bytes = 0;
@@ -228,6 +232,22 @@ int group_canonical(bs_op* op, const u64* hx, const u64* hz, const double* hc, i
     BS_COUNT_LAUNCH(5);
     BS_CUDA(cudaGetLastError());
     return finish_op(op, xc.p, cc.p, st);
+}
+
+namespace {
+
+int group_canonical(bs_op* op, const u64* hx, const u64* hz, const double* hc, i64 M0, double eps, cudaStream_t st) {
+    DevBuf<u64> x0, z0;
+    DevBuf<double2> c0;
+    BS_CUDA(x0.alloc(M0));
+    BS_CUDA(z0.alloc(M0));
+    BS_CUDA(c0.alloc(M0));
+    if (M0) {
+        BS_CUDA(cudaMemcpyAsync(x0.p, hx, M0 * 8, cudaMemcpyHostToDevice, st));
+        BS_CUDA(cudaMemcpyAsync(z0.p, hz, M0 * 8, cudaMemcpyHostToDevice, st));
+        BS_CUDA(cudaMemcpyAsync(c0.p, hc, M0 * 16, cudaMemcpyHostToDevice, st));
+    }
+    return bs_group_canonical_dev(op, x0.p, z0.p, c0.p, M0, eps, st);  // synchronises before the buffers die
 }
 
 int group_sequence(bs_op* op, const u64* hx, const u64* hz, const double* hc, i64 M, const i64* seq, i64 n_seq,
