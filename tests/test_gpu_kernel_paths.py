@@ -81,3 +81,34 @@ def test_kernel_path(env, kernel):
     e.update(env)
     r = subprocess.run([sys.executable, "-c", SCRIPT, ROOT, kernel], env=e, capture_output=True, text=True, timeout=900)
     assert r.returncode == 0 and "PATH OK" in r.stdout, r.stdout[-3000:] + r.stderr[-3000:]
+
+
+def test_wide_beta_space_uses_v1_fallback():
+    """D_beta > 32767 does not fit the u16 column tables: the v1 kernel must take over and stay exact."""
+    import numpy as np
+    import torch
+
+    import synth_inputs as si
+    from common import rel_l2
+    from oracle import oracle as orc
+    from paper_2606_28952_b200 import bs
+    L = 18
+    op = bs.bs_jw_hubbard(L, 1.0, 4.0)
+    ref = orc.hubbard_h(L, 1.0, 4.0)
+    sec, osec = bs.bs_sector_build(L, 1, 9), orc.Sector(L, 1, 9)
+    assert osec.dim_beta == 48620 and "sector_v1" in bs.bs_plan_describe(op, sec)
+    psi = si.random_state(osec.dim, 12)
+    want = osec.apply_grouped(ref, psi)
+    d_in = torch.from_numpy(psi).cuda()
+    d_out = torch.empty_like(d_in)
+    bs.bs_apply(op, sec, d_in, d_out)
+    assert rel_l2(d_out.cpu().numpy(), want) <= 1e-12
+    assert abs(bs.bs_expect(op, sec, d_in) - orc.vdot(psi, want)) <= 1e-10
+    # the mirrored sector (wide alpha space) also falls back
+    sec2, osec2 = bs.bs_sector_build(L, 9, 1), orc.Sector(L, 9, 1)
+    assert "sector_v1" in bs.bs_plan_describe(op, sec2)
+    psi2 = si.random_state(osec2.dim, 13)
+    d2 = torch.from_numpy(psi2).cuda()
+    o2 = torch.empty_like(d2)
+    bs.bs_apply(op, sec2, d2, o2)
+    assert rel_l2(o2.cpu().numpy(), osec2.apply_grouped(ref, psi2)) <= 1e-12
