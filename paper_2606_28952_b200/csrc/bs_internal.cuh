@@ -81,6 +81,17 @@ struct bs_op {
     DevBuf<i64> d_offs;
     DevBuf<double2> d_w;
     std::vector<u64> validated_sectors;  // sector ids this generator list was leak-checked against
+    // per sector id: for every generator the (row, partner row) pairs whose rotation this row owns (a6)
+    struct RotRows {
+        std::vector<i64> off;   // [G + 1]
+        DevBuf<uint2> d_pairs;  // {row, partner row}
+        DevBuf<double> d_th;    // thetas of the current call
+        DevBuf<double2> d_sc;   // (sin, cos) of the thetas
+    };
+    std::map<u64, RotRows*> rot_rows;
+    ~bs_op() {
+        for (auto& kv : rot_rows) delete kv.second;
+    }
 };
 
 // ---- sector ---------------------------------------------------------------------------------

@@ -71,6 +71,185 @@ k_rot_sector(SpinTab A, SpinTab B, int n_orb, u64 x, const u64* __restrict__ z, 
     rotate_pair(psi, i, iu, phase_sum(z, w, k0, k1, (u64)ta | ((u64)tb << n_orb)), theta, sc1);
 }
 
+// Row-list variant: the alpha side (validity, partner row, ownership) is precomputed per (generator, sector)
+// on the host, so the grid holds only rows that own pairs and the kernel's dependent chain is
+// beta string -> partner column -> amplitudes.
+__global__ void __launch_bounds__(256)
+k_rot_rows(SpinTab A, SpinTab B, int n_orb, u64 x, const uint2* __restrict__ pairs, const u64* __restrict__ z,
+           const double2* __restrict__ w, int k0, int k1, double theta, double2 sc1, double2* __restrict__ psi) {
+    const uint2 pr = __ldg(pairs + blockIdx.y);
+    const u32 row = pr.x, urow = pr.y, col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= B.D) return;
+    const u32 xb = (u32)(x >> n_orb);
+    const u32 ta = A.str[row], tb = B.str[col];
+    if (2 * __popc(tb & xb) != __popc(xb)) return;
+    const u32 ucol = xb ? spin_rank(B, tb ^ xb) : col;
+    if (urow == row && ucol < col) return;  // x_a = 0: the pair belongs to its smaller column
+    rotate_pair(psi, (i64)row * B.D + col, (i64)urow * B.D + ucol, phase_sum(z, w, k0, k1, (u64)ta | ((u64)tb << n_orb)),
+                theta, sc1);
+}
+
+// ---- closed-cell batching -------------------------------------------------------------------------------
+// A run of consecutive generators can share ONE launch when the index space splits into cells that are closed
+// under every pairing t <-> t ^ x_j of the run and fit in shared memory; inside a cell the rotations are applied
+// one after the other with __syncthreads() in between, outside they are independent:
+//   * all x_a equal (0 or not): cell = the row (x_a = 0) or the row pair {row, partner row}   (k_rot_cell_rows)
+//   * all x_b = 0:              cell = a few columns, all rows                                 (k_rot_cell_cols)
+// With the generator order of DESIGN.md reading U10 the 1,818 UCCSD rotations of config 2 become 40 launches.
+__device__ __forceinline__ void rotate_smem(double2& pa, double2& pb, double2 F, double theta, double2 sc1) {
+    const double r2 = F.x * F.x + F.y * F.y;
+    if (r2 == 0.0) return;
+    double sn = sc1.x, cs = sc1.y;
+    if (r2 != 1.0) {
+        const double r = hypot(F.x, F.y);
+        sincos(theta * r, &sn, &cs);
+        sn /= r;
+    }
+    const double2 a = pa, b = pb;
+    pa = make_double2(cs * a.x + sn * (F.x * b.x - F.y * b.y), cs * a.y + sn * (F.x * b.y + F.y * b.x));
+    pb = make_double2(cs * b.x - sn * (F.x * a.x + F.y * a.y), cs * b.y - sn * (F.x * a.y - F.y * a.x));
+}
+
+// Generator data of a chunk of the run, staged in shared memory by the whole block in one pass (all loads in
+// flight together) so that the serial generator loop never waits on global memory for its headers or strings.
+constexpr int kGenChunk = 32;   // generators per chunk
+constexpr int kStrChunk = 256;  // strings per chunk (a chunk ends early when they would not fit)
+struct GenChunk {
+    u64 z[kStrChunk];
+    double2 w[kStrChunk];
+    double2 sc[kGenChunk];
+    double th[kGenChunk];
+    u64 x[kGenChunk];
+    int k0[kGenChunk + 1];  // string offsets relative to the chunk
+    int n;                  // generators in the chunk
+};
+
+// loads generators [j, ...) into G; every thread returns the same chunk length
+__device__ __forceinline__ int load_chunk(GenChunk& G, i64 j, i64 j1, const u64* __restrict__ xg,
+                                          const i64* __restrict__ offs, const u64* __restrict__ z,
+                                          const double2* __restrict__ w, const double* __restrict__ thetas,
+                                          const double2* __restrict__ sc) {
+    const i64 base = offs[j];
+    int n = (int)min((i64)kGenChunk, j1 - j);
+    while (n > 1 && offs[j + n] - base > kStrChunk) --n;  // uniform
+    const int ns = (int)min((i64)kStrChunk, offs[j + n] - base);
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        G.x[i] = xg[j + i];
+        G.th[i] = thetas[j + i];
+        G.sc[i] = sc[j + i];
+    }
+    for (int i = threadIdx.x; i <= n; i += blockDim.x) G.k0[i] = (int)(offs[j + i] - base);
+    for (int i = threadIdx.x; i < ns; i += blockDim.x) {
+        G.z[i] = z[base + i];
+        G.w[i] = w[base + i];
+    }
+    if (threadIdx.x == 0) G.n = n;
+    return n;
+}
+
+__device__ __forceinline__ double2 phase_sum_s(const GenChunk& G, int k0, int k1, u64 t) {
+    double fr = 0.0, fi = 0.0;
+    for (int k = k0; k < k1; ++k) {
+        const u32 par = (u32)__popcll(G.z[k] & t) & 1u;
+        fr += flipd(G.w[k].x, par);
+        fi += flipd(G.w[k].y, par);
+    }
+    return make_double2(fr, fi);
+}
+
+// cells = rows (R = 1, x_a = 0) or row pairs (R = 2, common x_a != 0); generators [j0, j1)
+template <int R>
+__global__ void __launch_bounds__(R == 2 ? 512 : 256)
+k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
+                const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
+                const double* __restrict__ thetas, const double2* __restrict__ sc, i64 j0, i64 j1,
+                double2* __restrict__ psi) {
+    extern __shared__ __align__(16) unsigned char smem_cell[];
+    __shared__ GenChunk G;
+    double2* s0 = reinterpret_cast<double2*>(smem_cell);
+    const u32 Db = (u32)B.D;
+    double2* s1 = (R == 2) ? s0 + Db : s0;
+    u32 row0, row1;
+    if (R == 2) {
+        const uint2 pr = pairs[blockIdx.x];
+        row0 = pr.x;
+        row1 = pr.y;
+    } else row0 = row1 = blockIdx.x;
+    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
+        s0[c] = psi[(i64)row0 * Db + c];
+        if (R == 2) s1[c] = psi[(i64)row1 * Db + c];
+    }
+    const u32 ta = A.str[row0];
+    for (i64 j = j0; j < j1;) {
+        __syncthreads();  // previous chunk fully consumed (and the rows are loaded)
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        __syncthreads();
+        for (int g = 0; g < n; ++g) {
+            const u32 xb = (u32)(G.x[g] >> n_orb);
+            const u32 pxb = (u32)__popc(xb);
+            const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
+            for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
+                const u32 tb = B.str[c];
+                if (2u * (u32)__popc(tb & xb) != pxb) continue;
+                const u32 uc = xb ? spin_rank(B, tb ^ xb) : c;
+                if (R == 1 && uc <= c) continue;  // same row: the pair belongs to its smaller column (x_b != 0 here)
+                rotate_smem(s0[c], s1[uc], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)), G.th[g], G.sc[g]);
+            }
+            __syncthreads();
+        }
+        j += n;
+    }
+    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
+        psi[(i64)row0 * Db + c] = s0[c];
+        if (R == 2) psi[(i64)row1 * Db + c] = s1[c];
+    }
+}
+
+// cells = CC consecutive columns x all rows (x_b = 0 for every generator of the run)
+template <int CC>
+__global__ void __launch_bounds__(1024)
+k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, const i64* __restrict__ offs,
+                const u64* __restrict__ z, const double2* __restrict__ w, const double* __restrict__ thetas,
+                const double2* __restrict__ sc, i64 j0, i64 j1, double2* __restrict__ psi) {
+    extern __shared__ __align__(16) unsigned char smem_cell[];
+    __shared__ GenChunk G;
+    double2* sm = reinterpret_cast<double2*>(smem_cell);  // [Da][CC]
+    const u32 Da = (u32)A.D, Db = (u32)B.D;
+    const u32 c0 = blockIdx.x * CC;
+    const u32 ncol = min((u32)CC, Db - c0);
+    for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
+        const u32 r = i / CC, c = i - r * CC;
+        if (c < ncol) sm[i] = psi[(i64)r * Db + c0 + c];
+    }
+    const u64 mask_a = (u64(1) << n_orb) - 1;
+    for (i64 j = j0; j < j1;) {
+        __syncthreads();
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        __syncthreads();
+        for (int g = 0; g < n; ++g) {
+            const u32 xa = (u32)(G.x[g] & mask_a);
+            const u32 pxa = (u32)__popc(xa);
+            const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
+            for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
+                const u32 r = i / CC, c = i - r * CC;
+                if (c >= ncol) continue;
+                const u32 ta = A.str[r];
+                if (2u * (u32)__popc(ta & xa) != pxa) continue;
+                const u32 ur = spin_rank(A, ta ^ xa);
+                if (ur <= r) continue;  // x_a != 0: the pair belongs to its smaller row
+                const u32 tb = B.str[c0 + c];
+                rotate_smem(sm[i], sm[ur * CC + c], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)), G.th[g], G.sc[g]);
+            }
+            __syncthreads();
+        }
+        j += n;
+    }
+    for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
+        const u32 r = i / CC, c = i - r * CC;
+        if (c < ncol) psi[(i64)r * Db + c0 + c] = sm[i];
+    }
+}
+
 // One-off validation of a generator list against a sector: for every generator (blockIdx.y) and
 // every sector configuration t whose partner t^x lies outside the sector, F(t) must vanish;
 // otherwise exp(theta A) would leak out of the sector and its restriction would not be unitary.
@@ -148,18 +327,125 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
         BS_REQUIRE(!leak, BS_ERR_LEAVES_SECTOR, "a generator maps the sector outside itself");
         gen->validated_sectors.push_back(s->id);
     }
+    // owner-row lists of this (generators, sector) pair, built once on the host
+    bs_op::RotRows* RR = nullptr;
+    if (!s->full && (double)n_rot * (double)s->Da <= 5e8) {
+        auto it = gen->rot_rows.find(s->id);
+        if (it == gen->rot_rows.end()) {
+            RR = new (std::nothrow) bs_op::RotRows;
+            BS_REQUIRE(RR, BS_ERR_ALLOC, "bs_apply_pauli_rotations: host allocation failed");
+            std::vector<uint2> pairs;
+            RR->off.assign(n_rot + 1, 0);
+            const u64 mask_a = (u64(1) << s->n_orb) - 1;
+            for (i64 j = 0; j < n_rot; ++j) {
+                const u64 xa = gen->h_xg[j] & mask_a;
+                const int pxa = __builtin_popcountll(xa);
+                for (i64 r = 0; r < s->Da; ++r) {
+                    const u64 ta = s->h_sa[r];
+                    if (2 * __builtin_popcountll(ta & xa) != pxa) continue;
+                    const i64 ur = xa ? (i64)(std::lower_bound(s->h_sa.begin(), s->h_sa.end(), ta ^ xa) - s->h_sa.begin()) : r;
+                    if (ur >= r) pairs.push_back(make_uint2((u32)r, (u32)ur));
+                }
+                RR->off[j + 1] = (i64)pairs.size();
+            }
+            cudaError_t e = RR->d_pairs.upload(pairs, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) {
+                delete RR;
+                BS_CUDA(e);
+            }
+            gen->rot_rows[s->id] = RR;
+        } else RR = it->second;
+    }
     const dim3 sgrid((unsigned)((s->Db + 255) / 256), (unsigned)std::min<i64>(s->Da, 65535));
     BS_REQUIRE(s->full || s->Da <= 65535, BS_ERR_ARG, "bs_apply_pauli_rotations: more than 65535 alpha strings");
+    // ---- closed-cell batching of runs of generators (see k_rot_cell_rows) -------------------------------------
+    std::vector<char> done(n_rot, 0);
+    if (RR && !getenv("BS_ROT_PER_LAUNCH")) {
+        const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
+        const u64 mask_a = (u64(1) << s->n_orb) - 1;
+        std::vector<double2> h_sc(n_rot);
+        for (i64 j = 0; j < n_rot; ++j) h_sc[j] = make_double2(sin(thetas[j]), cos(thetas[j]));
+        if (RR->d_th.n < (size_t)n_rot) {
+            BS_CUDA(RR->d_th.alloc(n_rot));
+            BS_CUDA(RR->d_sc.alloc(n_rot));
+        }
+        BS_CUDA(cudaMemcpyAsync(RR->d_th.p, thetas, n_rot * 8, cudaMemcpyHostToDevice, st));
+        BS_CUDA(cudaMemcpyAsync(RR->d_sc.p, h_sc.data(), n_rot * 16, cudaMemcpyHostToDevice, st));
+        BS_CUDA(cudaStreamSynchronize(st));  // h_sc is a local
+        i64 j = 0;
+        while (j < n_rot) {
+            const u64 xa0 = gen->h_xg[j] & mask_a, xb0 = gen->h_xg[j] >> s->n_orb;
+            i64 e = j + 1;
+            int kind = 0;  // 1: common x_a (rows / row pairs), 2: all x_b = 0 (columns)
+            while (e < n_rot && (gen->h_xg[e] & mask_a) == xa0) ++e;
+            if (e - j >= 2) kind = 1;
+            else if (xb0 == 0) {
+                e = j + 1;
+                while (e < n_rot && (gen->h_xg[e] >> s->n_orb) == 0) ++e;
+                if (e - j >= 2) kind = 2;
+            }
+            for (i64 q = j; q < e && kind; ++q)
+                if (gen->h_offs[q + 1] - gen->h_offs[q] > 256) kind = 0;  // kStrChunk
+            if (kind == 1) {
+                const int R = xa0 ? 2 : 1;
+                const size_t smem = (size_t)R * s->Db * 16;
+                const i64 n_cells = xa0 ? RR->off[j + 1] - RR->off[j] : s->Da;
+                if (smem <= smem_cap && n_cells > 0) {
+                    const uint2* pr = RR->d_pairs.p + RR->off[j];
+                    if (R == 2) {
+                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                        k_rot_cell_rows<2><<<(unsigned)n_cells, 512, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
+                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                    } else {
+                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                        k_rot_cell_rows<1><<<(unsigned)n_cells, 256, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
+                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                    }
+                    BS_COUNT_LAUNCH(1);
+                    for (i64 q = j; q < e; ++q) done[q] = 1;
+                } else if (n_cells == 0) {
+                    for (i64 q = j; q < e; ++q) done[q] = 1;  // x_a never valid in this sector: identity
+                }
+            } else if (kind == 2) {
+                const int CC = ((size_t)s->Da * 8 * 16 <= smem_cap) ? 8 : (((size_t)s->Da * 2 * 16 <= smem_cap) ? 2 : 0);
+                if (CC) {
+                    const size_t smem = (size_t)s->Da * CC * 16;
+                    const unsigned nblk = (unsigned)((s->Db + CC - 1) / CC);
+                    if (CC == 8) {
+                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                        k_rot_cell_cols<8><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
+                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                    } else {
+                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                        k_rot_cell_cols<2><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
+                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                    }
+                    BS_COUNT_LAUNCH(1);
+                    for (i64 q = j; q < e; ++q) done[q] = 1;
+                }
+            }
+            j = e;
+        }
+    }
     for (i64 j = 0; j < n_rot; ++j) {
+        if (done[j]) continue;
         const int k0 = (int)gen->h_offs[j], k1 = (int)gen->h_offs[j + 1];
         const double2 sc1 = make_double2(sin(thetas[j]), cos(thetas[j]));
         if (s->full)
             k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
-        else
+        else if (RR) {
+            const i64 nr = RR->off[j + 1] - RR->off[j];
+            for (i64 r0 = 0; r0 < nr; r0 += 65535) {
+                const dim3 rg(sgrid.x, (unsigned)std::min<i64>(65535, nr - r0));
+                k_rot_rows<<<rg, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], RR->d_pairs.p + RR->off[j] + r0,
+                                               gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
+            }
+        } else
             k_rot_sector<<<sgrid, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1,
                                                 thetas[j], sc1, psi);
     }
-    BS_COUNT_LAUNCH(n_rot);
+    for (i64 j = 0; j < n_rot; ++j) BS_COUNT_LAUNCH(done[j] ? 0 : 1);
     BS_CUDA(cudaGetLastError());
     return BS_OK;
 }
