@@ -360,11 +360,30 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     const dim3 sgrid((unsigned)((s->Db + 255) / 256), (unsigned)std::min<i64>(s->Da, 65535));
     BS_REQUIRE(s->full || s->Da <= 65535, BS_ERR_ARG, "bs_apply_pauli_rotations: more than 65535 alpha strings");
     // ---- closed-cell batching of runs of generators (see k_rot_cell_rows) -------------------------------------
-    std::vector<char> done(n_rot, 0);
-    if (RR && !getenv("BS_ROT_PER_LAUNCH")) {
+    // one generator, one launch (isolated generators, cells too large for shared memory, full space)
+    auto single = [&](i64 j) {
+        const int k0 = (int)gen->h_offs[j], k1 = (int)gen->h_offs[j + 1];
+        const double2 sc1 = make_double2(sin(thetas[j]), cos(thetas[j]));
+        if (s->full)
+            k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
+        else if (RR) {
+            const i64 nr = RR->off[j + 1] - RR->off[j];
+            for (i64 r0 = 0; r0 < nr; r0 += 65535) {
+                const dim3 rg(sgrid.x, (unsigned)std::min<i64>(65535, nr - r0));
+                k_rot_rows<<<rg, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], RR->d_pairs.p + RR->off[j] + r0,
+                                               gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
+            }
+        } else
+            k_rot_sector<<<sgrid, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1,
+                                                thetas[j], sc1, psi);
+        BS_COUNT_LAUNCH(1);
+    };
+    const bool batching = RR && !getenv("BS_ROT_PER_LAUNCH");
+    {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
         const u64 mask_a = (u64(1) << s->n_orb) - 1;
-        std::vector<double2> h_sc(n_rot);
+        std::vector<double2> h_sc(batching ? n_rot : 0);
+        if (batching) {
         for (i64 j = 0; j < n_rot; ++j) h_sc[j] = make_double2(sin(thetas[j]), cos(thetas[j]));
         if (RR->d_th.n < (size_t)n_rot) {
             BS_CUDA(RR->d_th.alloc(n_rot));
@@ -373,14 +392,16 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
         BS_CUDA(cudaMemcpyAsync(RR->d_th.p, thetas, n_rot * 8, cudaMemcpyHostToDevice, st));
         BS_CUDA(cudaMemcpyAsync(RR->d_sc.p, h_sc.data(), n_rot * 16, cudaMemcpyHostToDevice, st));
         BS_CUDA(cudaStreamSynchronize(st));  // h_sc is a local
+        }
         i64 j = 0;
         while (j < n_rot) {
             const u64 xa0 = gen->h_xg[j] & mask_a, xb0 = gen->h_xg[j] >> s->n_orb;
             i64 e = j + 1;
             int kind = 0;  // 1: common x_a (rows / row pairs), 2: all x_b = 0 (columns)
-            while (e < n_rot && (gen->h_xg[e] & mask_a) == xa0) ++e;
+            bool launched = false;
+            while (batching && e < n_rot && (gen->h_xg[e] & mask_a) == xa0) ++e;
             if (e - j >= 2) kind = 1;
-            else if (xb0 == 0) {
+            else if (batching && xb0 == 0) {
                 e = j + 1;
                 while (e < n_rot && (gen->h_xg[e] >> s->n_orb) == 0) ++e;
                 if (e - j >= 2) kind = 2;
@@ -403,9 +424,9 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                             gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
                     }
                     BS_COUNT_LAUNCH(1);
-                    for (i64 q = j; q < e; ++q) done[q] = 1;
+                    launched = true;
                 } else if (n_cells == 0) {
-                    for (i64 q = j; q < e; ++q) done[q] = 1;  // x_a never valid in this sector: identity
+                    launched = true;  // x_a never valid in this sector: identity
                 }
             } else if (kind == 2) {
                 const int CC = ((size_t)s->Da * 8 * 16 <= smem_cap) ? 8 : (((size_t)s->Da * 2 * 16 <= smem_cap) ? 2 : 0);
@@ -422,30 +443,14 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                             gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
                     }
                     BS_COUNT_LAUNCH(1);
-                    for (i64 q = j; q < e; ++q) done[q] = 1;
+                    launched = true;
                 }
             }
+            if (!launched)
+                for (i64 q = j; q < e; ++q) single(q);  // in order: rotations do not commute
             j = e;
         }
     }
-    for (i64 j = 0; j < n_rot; ++j) {
-        if (done[j]) continue;
-        const int k0 = (int)gen->h_offs[j], k1 = (int)gen->h_offs[j + 1];
-        const double2 sc1 = make_double2(sin(thetas[j]), cos(thetas[j]));
-        if (s->full)
-            k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
-        else if (RR) {
-            const i64 nr = RR->off[j + 1] - RR->off[j];
-            for (i64 r0 = 0; r0 < nr; r0 += 65535) {
-                const dim3 rg(sgrid.x, (unsigned)std::min<i64>(65535, nr - r0));
-                k_rot_rows<<<rg, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], RR->d_pairs.p + RR->off[j] + r0,
-                                               gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
-            }
-        } else
-            k_rot_sector<<<sgrid, 256, 0, st>>>(s->ta, s->tb, s->n_orb, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1,
-                                                thetas[j], sc1, psi);
-    }
-    for (i64 j = 0; j < n_rot; ++j) BS_COUNT_LAUNCH(done[j] ? 0 : 1);
     BS_CUDA(cudaGetLastError());
     return BS_OK;
 }

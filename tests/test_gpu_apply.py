@@ -280,3 +280,49 @@ def test_q28_hubbard_single_apply(bs, orc):
     e = bs.bs_expect(op, sec, d_psi)
     assert abs(e - orc.vdot(psi, want)) <= TOL_E
     assert abs(e.real - 14.0) < 0.1                         # Tr H / D = U N_a N_b / L = 14 (pin P10)
+
+
+def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
+    """Shuffled generator order breaks the runs that the closed-cell batching relies on: isolated generators take
+    the per-generator kernel, short runs the cell kernels; BS_ROT_PER_LAUNCH=1 forces the per-generator path for
+    the ordered list.  All must agree with the fermionic Givens oracle."""
+    import os
+    import subprocess
+    import sys
+    from paper_2606_28952_b200 import jw_terms as jw
+    ex = si.uccsd_excitations(7, 3, 4)
+    rng = np.random.default_rng(21)
+    order = rng.permutation(len(ex))
+    ex_s = [ex[i] for i in order]
+    th = si.thetas(len(ex_s), 9, sd=0.3)
+    X, Z, Cc, offs = jw.excitation_generator_terms(ex_s)
+    gens = bs.bs_group_xmask(X, Z, Cc, 14, 0.0, bs.BS_MODE_SEQUENCE, offs)
+    osec, sec = orc.Sector(7, 3, 4), bs.bs_sector_build(7, 3, 4)
+    psi = si.random_state(osec.dim, 2)
+    d = to_device(psi)
+    bs.bs_apply_pauli_rotations(gens, sec, th, d)
+    for (cre, ann), t in zip(ex_s, th):
+        osec.rot_fermionic(psi, cre, ann, t)
+    assert rel_l2(to_host(d), psi) <= TOL_L2
+    code = (
+        "import sys, os; sys.path.insert(0, sys.argv[1]); sys.path.insert(0, os.path.join(sys.argv[1], 'tests'))\n"
+        "import numpy as np, torch, synth_inputs as si\n"
+        "from oracle import oracle as orc\n"
+        "from paper_2606_28952_b200 import bs, jw_terms as jw\n"
+        "ex = si.uccsd_excitations(6, 3, 3); th = si.thetas(len(ex), 5, sd=0.4)\n"
+        "X, Z, C, offs = jw.excitation_generator_terms(ex)\n"
+        "g = bs.bs_group_xmask(X, Z, C, 12, 0.0, bs.BS_MODE_SEQUENCE, offs)\n"
+        "sec, osec = bs.bs_sector_build(6, 3, 3), orc.Sector(6, 3, 3)\n"
+        "psi = si.random_state(400, 8); d = torch.from_numpy(psi.copy()).cuda()\n"
+        "n0 = bs.bs_launch_count(); bs.bs_apply_pauli_rotations(g, sec, th, d); n1 = bs.bs_launch_count()\n"
+        "for (cre, ann), t in zip(ex, th): osec.rot_fermionic(psi, cre, ann, t)\n"
+        "err = np.linalg.norm(d.cpu().numpy() - psi) / np.linalg.norm(psi)\n"
+        "print('LAUNCHES', n1 - n0, 'ERR', err); assert err <= 1e-12\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    counts = {}
+    for env in ({}, {"BS_ROT_PER_LAUNCH": "1"}):
+        r = subprocess.run([sys.executable, "-c", code, root], env=dict(os.environ, **env), capture_output=True,
+                           text=True, timeout=600)
+        assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+        counts[bool(env)] = int(r.stdout.split("LAUNCHES")[1].split()[0])
+    assert counts[True] > 3 * counts[False]      # batching really reduces the launch count
