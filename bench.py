@@ -144,6 +144,12 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
            "raw_terms": m_raw, "setup_s": round(t_setup, 3),
            "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
            "l2_flush_between_reps": bool(flush)}
+    if cfg.kind == "molecular":       # non-zeros per row of H in the sector for generic integrals
+        from math import comb
+        oa, va, ob, vb = cfg.n_alpha, cfg.n_orb - cfg.n_alpha, cfg.n_beta, cfg.n_orb - cfg.n_beta
+        nnz_row = 1 + oa * va + ob * vb + comb(oa, 2) * comb(va, 2) + comb(ob, 2) * comb(vb, 2) + oa * va * ob * vb
+        ent["nonzeros_per_s"] = nnz_row * cfg.dim / (apply_ms * 1e-3)
+        ent["gather_gbs"] = 16 * ent["nonzeros_per_s"] / 1e9      # 16-byte amplitude gathers through L2 / shared memory
     bytes_alg = 32 * cfg.dim + table_bytes(op)
     ent["hbm_gbs_algorithmic"] = bytes_alg / apply_ms / 1e6
     ent["hbm_frac_of_measured_peak"] = ent["hbm_gbs_algorithmic"] / peak_gbs
