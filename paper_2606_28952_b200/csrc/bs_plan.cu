@@ -126,6 +126,8 @@ int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
         return a.xa < b.xa || (a.xa == b.xa && a.xb < b.xb);
     });
     build_row_plans(P, groups, S, st);
+    P->real_w = real_w;
+    if (P->rp_main) return BS_OK;  // the v1 tables below are only needed when the v2 row plan could not be built
     std::vector<u32> xa_list, ga_off;
     std::vector<uint4> hdr;
     std::vector<uint2> szab;
