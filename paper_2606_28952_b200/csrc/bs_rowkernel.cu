@@ -1,18 +1,19 @@
 // a4 apply, v2 row kernel (Eq. 27; Eq. 28).
 //
-// One thread block owns one target row t_a and a chunk of target columns t_b; every thread owns up
-// to CPT columns and keeps their accumulators in registers.  For every alpha mask x_a that is valid
-// for the row (precomputed list: mask id, source row) the block
-//   1. evaluates the row-dependent phase factors V_gj(t_a) of all groups under x_a into shared
-//      memory (one per KEY = distinct beta Z mask of a group; strings are visited once per row, not
-//      once per target),
-//   2. if some group under x_a moves the beta string, stages the source row psi[u_a, :] in shared
-//      memory with TMA bulk copies (cp.async.bulk + mbarrier), in windows if the row is larger than
-//      shared memory,
-//   3. walks the groups: one coalesced u16 load from the column table gives validity, source column
-//      and the first sign; remaining keys cost one AND + bit test (or POPC) + sign flip + add; the
-//      source amplitude is a 128-bit shared-memory gather (x_b != 0) or a coalesced 128-bit global
-//      load (x_b = 0: same column of another row), then two (real V) or four FMAs.
+// One thread block owns one target row t_a and a chunk of target columns t_b; every thread owns CPT
+// columns (stride = blockDim, so global accesses coalesce) and keeps their accumulators in registers.
+// The row's valid alpha masks (precomputed list: mask id, source row, V-slot offset) are processed in
+// batches -- one staged entry, or a run of alpha-only entries whose keys fit the V slots:
+//   1. phase factors V_gj(t_a) of every key (= distinct beta Z mask of a group) of the batch go to shared
+//      memory, one warp per entry, one lane per key: strings are visited once per row, not once per target;
+//   2. a staged entry (some group moves the beta string) gets its source row psi[u_a, :] by TMA bulk copies
+//      (cp.async.bulk + mbarrier), in windows if the row is larger than shared memory;
+//   3. "simple" entries (one group, x_b = 0, one key) are row axpys with coalesced 128-bit loads; general
+//      groups read 4 packed u16 table entries per thread (validity, source column, first sign), add the
+//      remaining keys (bit-shift sign for single-bit Z masks, POPC otherwise) and gather the amplitude from
+//      the staged row (LDS.128) or from global memory;
+//   4. the column-list pass serves all single-key x_b != 0 groups of the entry from a per-column compacted
+//      list (no invalid lanes, no branches): V from shared memory by table id, amplitude by LDS.128.
 // No tensor cores: this is a gather with integer bit math (north star).
 #include <algorithm>
 
