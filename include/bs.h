@@ -27,6 +27,10 @@
  * thread-local message.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default
  * stream); kernels are enqueued on it and the call returns without synchronising unless stated.
  * There is NO CPU fallback: without a CUDA device every compute entry point returns BS_ERR_CUDA.
+ *
+ * Threading: handles may be shared between host threads, but calls that use the same (operator, sector) pair
+ * share library-owned scratch (cached plan, transposed copies, reduction partials) and must be issued on one
+ * stream at a time.  Different pairs are independent.
  */
 #ifndef BS_H_
 #define BS_H_
