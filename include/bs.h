@@ -120,8 +120,9 @@ int bs_expect(bs_op_t op, bs_sector_t s, const void* psi, double result_reim[2],
 int bs_vdot(bs_sector_t s, const void* a, const void* b, double result_reim[2], void* cuda_stream);
 
 /* ---- a6: psi <- exp(theta_j A_j) psi for j = 0..n_rot-1 in order, A_j = group j of a
- * BS_MODE_SEQUENCE operator: anti-Hermitian (every c_k purely imaginary), one x != 0, mutually
- * commuting strings (Eq. 39).  thetas [host] double[n_rot], n_rot must
+ * BS_MODE_SEQUENCE operator: anti-Hermitian (every c_k purely imaginary), one x, mutually
+ * commuting strings (Eq. 39).  x = 0 (diagonal generator, e.g. exp(-i w Z_j Z_{j+1}) of
+ * PAPER.md:469-473, Eq. 42) multiplies every amplitude by exp(theta F(t)).  thetas [host] double[n_rot], n_rot must
  * equal the operator's group count.  In place on disjoint pairs {t, t^x}.  Returns
  * BS_ERR_NOT_COMMUTING / BS_ERR_LEAVES_SECTOR instead of applying a non-unitary map.
  * The first call for a (generators, sector) pair runs a read-only leak check and synchronises; later

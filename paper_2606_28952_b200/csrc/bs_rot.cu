@@ -1,6 +1,6 @@
 // a6 grouped Pauli rotations (section 2.5; Eq. 39).
 //
-// Generator A = sum_k c_k P_k, all strings sharing one x != 0 and mutually commuting, A^dag = -A.
+// Generator A = sum_k c_k P_k, all strings sharing one x and mutually commuting, A^dag = -A (x = 0: k_rot_diag).
 // With F(t) = sum_k w_k (-1)^{popc(z_k & t)} = <t|A|t^x> (target form, w_k = c_k (-i)^{ny_k}) the
 // operator is block diagonal on the pairs {t, u = t^x}: A|u> = F(t)|t>, A|t> = F(u)|u>,
 // F(u) = -conj F(t), A^2 = -|F|^2 on the pair, hence
@@ -87,6 +87,26 @@ k_rot_rows(SpinTab A, SpinTab B, int n_orb, u64 x, const uint2* __restrict__ pai
     if (urow == row && ucol < col) return;  // x_a = 0: the pair belongs to its smaller column
     rotate_pair(psi, (i64)row * B.D + col, (i64)urow * B.D + ucol, phase_sum(z, w, k0, k1, (u64)ta | ((u64)tb << n_orb)),
                 theta, sc1);
+}
+
+// Diagonal generator (x = 0, e.g. exp(-i w Z_j Z_{j+1}) of the layered TFIM ansatz, Eq. 42):
+// A|t> = F(t)|t> with F purely imaginary for an anti-Hermitian A, so psi[t] *= exp(theta F(t)).
+__global__ void __launch_bounds__(256)
+k_rot_diag(SpinTab A, SpinTab B, int n_orb, int full, i64 D, const u64* __restrict__ z, const double2* __restrict__ w,
+           int k0, int k1, double theta, double2* __restrict__ psi) {
+    const i64 i = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (i >= D) return;
+    u64 t = (u64)i;
+    if (!full) {
+        const i64 row = i / B.D;
+        t = (u64)A.str[row] | ((u64)B.str[i - row * B.D] << n_orb);
+    }
+    const double2 F = phase_sum(z, w, k0, k1, t);
+    double sn, cs;
+    sincos(theta * F.y, &sn, &cs);
+    const double m = exp(theta * F.x);  // 1 for an anti-Hermitian generator
+    const double2 a = psi[i];
+    psi[i] = make_double2(m * (cs * a.x - sn * a.y), m * (cs * a.y + sn * a.x));
 }
 
 // ---- closed-cell batching -------------------------------------------------------------------------------
@@ -292,11 +312,9 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     BS_REQUIRE(n_rot == 0 || thetas, BS_ERR_ARG, "bs_apply_pauli_rotations: thetas is NULL");
     BS_REQUIRE(psi_inout && (reinterpret_cast<uintptr_t>(psi_inout) & 15u) == 0, BS_ERR_ARG,
                "psi is NULL or not 16-byte aligned");
-    // validation: x != 0, anti-Hermitian (c purely imaginary), mutually commuting (equal ny parity)
+    // validation: anti-Hermitian (c purely imaginary), mutually commuting (equal ny parity)
     for (i64 j = 0; j < gen->G; ++j) {
         const u64 x = gen->h_xg[j];
-        BS_REQUIRE(x != 0, BS_ERR_ARG, "generator %lld has x = 0 (diagonal generators are not rotations of pairs)",
-                   (long long)j);
         int par0 = -1;
         for (i64 k = gen->h_offs[j]; k < gen->h_offs[j + 1]; ++k) {
             const double re = gen->h_c[2 * k], im = gen->h_c[2 * k + 1];
@@ -364,7 +382,10 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     auto single = [&](i64 j) {
         const int k0 = (int)gen->h_offs[j], k1 = (int)gen->h_offs[j + 1];
         const double2 sc1 = make_double2(sin(thetas[j]), cos(thetas[j]));
-        if (s->full)
+        if (gen->h_xg[j] == 0)
+            k_rot_diag<<<nb, 256, 0, st>>>(s->ta, s->tb, s->n_orb, s->full ? 1 : 0, s->D, gen->d_z.p, gen->d_w.p, k0, k1,
+                                           thetas[j], psi);
+        else if (s->full)
             k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
         else if (RR) {
             const i64 nr = RR->off[j + 1] - RR->off[j];
@@ -399,11 +420,12 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
             i64 e = j + 1;
             int kind = 0;  // 1: common x_a (rows / row pairs), 2: all x_b = 0 (columns)
             bool launched = false;
-            while (batching && e < n_rot && (gen->h_xg[e] & mask_a) == xa0) ++e;
+            const bool diag0 = gen->h_xg[j] == 0;  // diagonal generators never join a run
+            while (batching && !diag0 && e < n_rot && gen->h_xg[e] != 0 && (gen->h_xg[e] & mask_a) == xa0) ++e;
             if (e - j >= 2) kind = 1;
-            else if (batching && xb0 == 0) {
+            else if (batching && !diag0 && xb0 == 0) {
                 e = j + 1;
-                while (e < n_rot && (gen->h_xg[e] >> s->n_orb) == 0) ++e;
+                while (e < n_rot && gen->h_xg[e] != 0 && (gen->h_xg[e] >> s->n_orb) == 0) ++e;
                 if (e - j >= 2) kind = 2;
             }
             for (i64 q = j; q < e && kind; ++q)
