@@ -177,6 +177,17 @@ __device__ __forceinline__ double2 phase_sum_s(const GenChunk& G, int k0, int k1
     return make_double2(fr, fi);
 }
 
+// beta-only phase sum: the alpha half of every sign was folded into G.w for this block's row (see fold below)
+__device__ __forceinline__ double2 phase_sum_b(const GenChunk& G, int k0, int k1, u32 tb) {
+    double fr = 0.0, fi = 0.0;
+    for (int k = k0; k < k1; ++k) {
+        const u32 par = (u32)__popc((u32)G.z[k] & tb) & 1u;
+        fr += flipd(G.w[k].x, par);
+        fi += flipd(G.w[k].y, par);
+    }
+    return make_double2(fr, fi);
+}
+
 // cells = rows (R = 1, x_a = 0) or row pairs (R = 2, common x_a != 0); generators [j0, j1)
 template <int R>
 __global__ void __launch_bounds__(R == 2 ? 512 : 256)
@@ -204,6 +215,15 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
         __syncthreads();  // previous chunk fully consumed (and the rows are loaded)
         const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
         __syncthreads();
+        // fold the alpha half of every sign into the weights (t_a is fixed for the block): the per-column phase
+        // sum is then one 32-bit AND + POPC per string
+        for (int i = threadIdx.x; i < min(G.k0[n], kStrChunk); i += blockDim.x) {
+            const u64 zz = G.z[i];
+            const u32 par = (u32)__popc((u32)(zz & ((u64(1) << n_orb) - 1)) & ta) & 1u;
+            G.w[i] = make_double2(flipd(G.w[i].x, par), flipd(G.w[i].y, par));
+            G.z[i] = zz >> n_orb;
+        }
+        __syncthreads();
         for (int g = 0; g < n; ++g) {
             const u32 xb = (u32)(G.x[g] >> n_orb);
             const u32 pxb = (u32)__popc(xb);
@@ -213,7 +233,7 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
                 if (2u * (u32)__popc(tb & xb) != pxb) continue;
                 const u32 uc = xb ? spin_rank(B, tb ^ xb) : c;
                 if (R == 1 && uc <= c) continue;  // same row: the pair belongs to its smaller column (x_b != 0 here)
-                rotate_smem(s0[c], s1[uc], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)), G.th[g], G.sc[g]);
+                rotate_smem(s0[c], s1[uc], phase_sum_b(G, k0, k1, tb), G.th[g], G.sc[g]);
             }
             __syncthreads();
         }
