@@ -326,3 +326,42 @@ def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
         counts[bool(env)] = int(r.stdout.split("LAUNCHES")[1].split()[0])
     assert counts[True] > 3 * counts[False]      # batching really reduces the launch count
+
+
+def test_apply_and_rotations_are_bit_reproducible(bs):
+    """No floating-point atomics and a fixed summation order: repeated runs give identical bits (a shared-memory or
+    global-memory race in the row kernel or the rotation cell kernels would show up here as run-to-run noise)."""
+    import torch
+    from paper_2606_28952_b200 import jw_terms as jw
+    cfg = si.CONFIGS["q24"]
+    op = _gpu_op(bs, "q24")
+    sec = bs.bs_sector_build(12, 6, 6)
+    d_in = to_device(si.random_state(cfg.dim, 17))
+    ref_out = torch.empty_like(d_in)
+    bs.bs_apply(op, sec, d_in, ref_out)
+    out = torch.empty_like(d_in)
+    for _ in range(10):
+        out.fill_(float("nan"))
+        bs.bs_apply(op, sec, d_in, out)
+        assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref_out))
+    ex = si.uccsd_excitations(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    th = si.thetas(len(ex), cfg.seed_theta)
+    X, Z, Cc, offs = jw.excitation_generator_terms(ex)
+    gens = bs.bs_group_xmask(X, Z, Cc, 24, 0.0, bs.BS_MODE_SEQUENCE, offs)
+    states = []
+    for _ in range(4):
+        psi = torch.zeros(cfg.dim, dtype=torch.complex128, device="cuda")
+        psi[0] = 1.0
+        bs.bs_apply_pauli_rotations(gens, sec, th, psi)
+        states.append(psi)
+    for s in states[1:]:
+        assert torch.equal(torch.view_as_real(s), torch.view_as_real(states[0]))
+    hub = bs.bs_jw_hubbard(10, 1.0, 4.0)
+    hsec = bs.bs_sector_build(10, 5, 5)
+    hin = to_device(si.random_state(hsec.dim, 3))
+    h0 = torch.empty_like(hin)
+    bs.bs_apply(hub, hsec, hin, h0)
+    for _ in range(10):
+        h1 = torch.empty_like(hin)
+        bs.bs_apply(hub, hsec, hin, h1)
+        assert torch.equal(torch.view_as_real(h1), torch.view_as_real(h0))
