@@ -76,6 +76,7 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
         bs_rowplan_free(t);
         return;
     }
+    if (!t && bs_light_build(m, st) != BS_OK) cudaGetLastError();  // optional fast path; k_rows stays available
     P->rp_main = m;
     P->rp_t = t;
 }
@@ -263,9 +264,9 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
         const bs_rowplan* M = P->rp_main;
         const bs_rowplan* T = P->rp_t;
         int w = snprintf(buf, (size_t)n,
-                         "kernel=rows_v2 real_w=%d main{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d "
+                         "kernel=rows_v2%s real_w=%d main{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d "
                          "row_ent=%lld threads=%d cpt=%d chunk_cols=%d win_cols=%d n_win=%d smem=%zu listed=%d l_max=%d}",
-                         (int)M->real_w, M->n_xa, (long long)M->n_items, (long long)M->n_keys, (long long)M->n_strings,
+                         M->light ? "+light" : "", (int)M->real_w, M->n_xa, (long long)M->n_items, (long long)M->n_keys, (long long)M->n_strings,
                          (long long)M->n_tkeys, M->max_keys, (long long)M->n_row_ent, M->threads, M->cpt, M->chunk_cols,
                          M->win_cols, M->n_win, M->smem, M->n_listed, M->l_max);
         if (T && w > 0 && w < n)

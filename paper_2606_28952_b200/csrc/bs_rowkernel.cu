@@ -444,11 +444,26 @@ cudaError_t launch_k_rows(const bs_rowplan* R, cudaStream_t st, const double2* p
 
 }  // namespace
 
+int bs_light_apply(bs_rowplan* R, const double2* psi, double2* out, i64 lo, i64 hi, const Epilogue& ep, bool expect,
+                   cudaStream_t st, double2* partials, i64* n_partials);
+
 // Runs the v2 path for rows [lo, hi).  expect: dot partials instead of stores.
 int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i64 lo, i64 hi, const Epilogue& ep,
                   bool expect, cudaStream_t st, i64* n_partials_out, double2** partials_out) {
     bs_rowplan* M = P->rp_main;
     const i64 Da = s->Da, Db = s->Db;
+    if (!P->rp_t && M->light) {
+        if (expect && P->n_partials < 1024) {
+            BS_CUDA(P->d_partials.alloc(1024));
+            P->n_partials = 1024;
+        }
+        i64 np = 0;
+        int rc = bs_light_apply(M, psi, out, lo, hi, ep, expect, st, P->d_partials.p, &np);
+        if (rc != BS_OK) return rc;
+        if (n_partials_out) *n_partials_out = expect ? np : 0;
+        if (partials_out) *partials_out = P->d_partials.p;
+        return BS_OK;
+    }
     if (!P->rp_t) {
         const i64 nblk = (hi - lo) * ((Db + M->chunk_cols - 1) / M->chunk_cols);
         if (expect && P->n_partials < nblk) {

@@ -263,6 +263,10 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     }
     // column list: compaction of the listed tables over table ids
     R->n_listed = n_listed;
+    R->h_hdrs = hdrs;
+    R->h_items = items;
+    R->h_tkeys = tkeys;
+    R->h_xa = xa_list;
     R->l_max = 0;
     if (n_listed > 0) {
         DevBuf<int> lcnt;

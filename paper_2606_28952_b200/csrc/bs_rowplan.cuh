@@ -77,4 +77,30 @@ struct bs_rowplan {
     int threads = 256, cpt = 1, n_chunks = 1, chunk_cols = 0, win_cols = 0, n_win = 1;
     size_t smem = 0;
     RowPlanDev dev{};
+    // host copies kept for the light-plan builder (bs_light.cu)
+    std::vector<XaHdr> h_hdrs;
+    std::vector<RowItem> h_items;
+    std::vector<uint2> h_tkeys;  // {xb, zb0} of every column table, listed ones first
+    std::vector<u32> h_xa;
+    // ---- light path (bs_light.cu): few groups, HBM-bound operators such as lattice models ---------------------
+    // One 1024-thread block per SM owns ALL columns of a strip of rows: the per-column hop list (u16 entries) lives
+    // in shared memory for the whole launch, rows are double-buffered by TMA, and every phase factor V(t_a) is
+    // precomputed per (row, key) at plan time, so the row loop has no V phase and no list traffic.
+    bool light = false;
+    int light_lmax = 0;
+    size_t light_smem = 0;
+    DevBuf<unsigned short> d_llist;  // [light_lmax][4096], slot s of thread t: column t + 1024 * (s & 3) ...
+    DevBuf<double> d_vtab;           // V values, row after row
+    DevBuf<i64> d_voff;              // [Da + 1]
 };
+
+struct LightDev {
+    RowPlanDev P;
+    const unsigned short* llist;
+    const double* vtab;
+    const i64* voff;
+    int l_max;
+    u32 item0, item_split, key0, key_split;  // of the x_a = 0 header
+    int lut_nq;                              // nibble tables of the diagonal (0: generic key loop)
+};
+int bs_light_build(bs_rowplan* R, cudaStream_t st);
