@@ -156,6 +156,11 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
             double2 acc[kLC];
 #pragma unroll
             for (int k = 0; k < kLC; ++k) acc[k] = make_double2(0.0, 0.0);
+            if (MODE == 0 && ep.acc) {  // the fused-axpy epilogue will read the accumulator: pull its lines into L2 now
+#pragma unroll
+                for (int k = 0; k < kLC; ++k)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ep.acc + r * (i64)Db + col[k]));
+            }
             if (L.lut_nq) {
                 if (r + rs < r1) build_lut(r + rs, b ^ 1u);  // visible after the barrier that ends this row
                 const double* __restrict__ lut = slut + b * 128;
