@@ -350,7 +350,8 @@ def run_ours(args):
             "e2e": {"value": world * applies_per_step * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 16 * D, "d2h_bytes_per_step": 16 * D + 16, "steps": e2e_steps,
                     "pipeline": "H2D of step i+1 and D2H of step i-1 overlap step i (2 device buffers, 3 streams)"},
-            "roofline": {"bound": "hbm", "kernel": "k_rows<MODE_FINAL> (fused apply+axpy launches of bs_taylor_step)",
+            "roofline": {"bound": "hbm", "kernel": ("k_light<0>" if "+light" in bs.bs_plan_describe(op, sec) else "k_rows<MODE_FINAL>")
+                         + " (fused apply+axpy launches of bs_taylor_step)",
                          "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
                          "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
                          "launch_ms": launch_ms, "traffic": TRAFFIC_NCU.get(name)},
@@ -371,7 +372,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {"q28_hubbard": 1.0356e9}   # profiles/r01_v2_q28_k_rows_full.md, fused apply+axpy launch
+TRAFFIC_NCU = {"q28_hubbard": 9.26e8}   # profiles/r01_v3_q28_k_light_full.md, fused apply+axpy launch
 
 
 def run_reference(args):
