@@ -365,3 +365,34 @@ def test_apply_and_rotations_are_bit_reproducible(bs):
         h1 = torch.empty_like(hin)
         bs.bs_apply(hub, hsec, hin, h1)
         assert torch.equal(torch.view_as_real(h1), torch.view_as_real(h0))
+
+
+def test_degenerate_operators_and_sectors(bs, orc):
+    """Empty operator, identity-only operator, one-dimensional sectors, fully occupied spin."""
+    import torch
+    e = np.zeros(0, np.uint64)
+    op_empty = bs.bs_group_xmask(e, e, np.zeros(0, np.complex128), 12)
+    op_id = bs.bs_group_xmask(np.zeros(1, np.uint64), np.zeros(1, np.uint64), np.array([2.5 - 1j]), 12)
+    ref = oracle_operator("q12")
+    op = _gpu_op(bs, "q12")
+    for (na, nb) in [(3, 3), (0, 0), (6, 6), (6, 0), (0, 1), (5, 6)]:
+        sec, osec = bs.bs_sector_build(6, na, nb), orc.Sector(6, na, nb)
+        psi = si.random_state(osec.dim, 50 + na + nb)
+        d_in = to_device(psi)
+        d_out = torch.full_like(d_in, complex(np.nan, np.nan))
+        bs.bs_apply(op_empty, sec, d_in, d_out)
+        assert np.all(to_host(d_out) == 0)
+        assert bs.bs_expect(op_empty, sec, d_in) == 0
+        bs.bs_apply(op_id, sec, d_in, d_out)
+        assert rel_l2(to_host(d_out), (2.5 - 1j) * psi) <= 1e-15
+        bs.bs_apply(op, sec, d_in, d_out)
+        want = osec.apply(ref, psi)
+        # (0,0) is the vacuum: H|vac> = 0 exactly and both sides return rounding residue of cancelling
+        # coefficients (~1e-15), so the error is measured against max(||want||, 1) there
+        assert np.linalg.norm(to_host(d_out) - want) <= TOL_L2 * max(np.linalg.norm(want), 1.0), (na, nb)
+        assert abs(bs.bs_expect(op, sec, d_in) - orc.vdot(psi, want)) <= TOL_E
+    full = bs.bs_sector_build(12)
+    d_in = to_device(si.random_state(4096, 1))
+    d_out = torch.full_like(d_in, 1.0)
+    bs.bs_apply(op_empty, full, d_in, d_out)
+    assert np.all(to_host(d_out) == 0)
