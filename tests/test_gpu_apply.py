@@ -396,3 +396,21 @@ def test_degenerate_operators_and_sectors(bs, orc):
     d_out = torch.full_like(d_in, 1.0)
     bs.bs_apply(op_empty, full, d_in, d_out)
     assert np.all(to_host(d_out) == 0)
+
+
+def test_rotations_on_degenerate_sectors(bs, orc):
+    """Number-conserving generators on sectors where no pair exists (full / empty spin) act as the identity; on a
+    half-empty sector only the generators of the populated spin act."""
+    from paper_2606_28952_b200 import jw_terms as jw
+    ex = si.uccsd_excitations(5, 2, 2)
+    th = si.thetas(len(ex), 77, sd=0.5)
+    X, Z, Cc, offs = jw.excitation_generator_terms(ex)
+    gens = bs.bs_group_xmask(X, Z, Cc, 10, 0.0, bs.BS_MODE_SEQUENCE, offs)
+    for (na, nb) in [(5, 5), (0, 0), (5, 0), (0, 3), (2, 5), (1, 4)]:
+        sec, osec = bs.bs_sector_build(5, na, nb), orc.Sector(5, na, nb)
+        psi = si.random_state(osec.dim, 9 + na + 7 * nb)
+        d = to_device(psi)
+        bs.bs_apply_pauli_rotations(gens, sec, th, d)
+        for (cre, ann), t in zip(ex, th):
+            osec.rot_fermionic(psi, cre, ann, t)
+        assert rel_l2(to_host(d), psi) <= TOL_L2, (na, nb)
