@@ -85,6 +85,9 @@ struct bs_op {
     struct RotRows {
         std::vector<i64> off;   // [G + 1]
         DevBuf<uint2> d_pairs;  // {row, partner row}
+        std::vector<i64> coff;  // [G + 1]
+        DevBuf<uint2> d_cpairs; // per generator the valid {column, partner column} pairs (x_a = 0: owner side only)
+        DevBuf<i64> d_off, d_coff;  // device copies of off / coff
         DevBuf<double> d_th;    // thetas of the current call
         DevBuf<double2> d_sc;   // (sin, cos) of the thetas
     };

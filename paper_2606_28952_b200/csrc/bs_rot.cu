@@ -193,8 +193,8 @@ template <int R>
 __global__ void __launch_bounds__(R == 2 ? 512 : 256)
 k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
                 const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
-                const double* __restrict__ thetas, const double2* __restrict__ sc, i64 j0, i64 j1,
-                double2* __restrict__ psi) {
+                const double* __restrict__ thetas, const double2* __restrict__ sc, const uint2* __restrict__ cpairs,
+                const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
     double2* s0 = reinterpret_cast<double2*>(smem_cell);
@@ -225,15 +225,13 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
         }
         __syncthreads();
         for (int g = 0; g < n; ++g) {
-            const u32 xb = (u32)(G.x[g] >> n_orb);
-            const u32 pxb = (u32)__popc(xb);
+            // the valid (column, partner column) pairs of the generator's beta mask were listed at plan time (they do
+            // not depend on the row): no validity test, no rank lookup, no idle lanes
             const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
-            for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
-                const u32 tb = B.str[c];
-                if (2u * (u32)__popc(tb & xb) != pxb) continue;
-                const u32 uc = xb ? spin_rank(B, tb ^ xb) : c;
-                if (R == 1 && uc <= c) continue;  // same row: the pair belongs to its smaller column (x_b != 0 here)
-                rotate_smem(s0[c], s1[uc], phase_sum_b(G, k0, k1, tb), G.th[g], G.sc[g]);
+            const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
+            for (i64 p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
+                const uint2 cp = __ldg(cpairs + p);
+                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, B.str[cp.x]), G.th[g], G.sc[g]);
             }
             __syncthreads();
         }
@@ -250,7 +248,8 @@ template <int CC>
 __global__ void __launch_bounds__(1024)
 k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, const i64* __restrict__ offs,
                 const u64* __restrict__ z, const double2* __restrict__ w, const double* __restrict__ thetas,
-                const double2* __restrict__ sc, i64 j0, i64 j1, double2* __restrict__ psi) {
+                const double2* __restrict__ sc, const uint2* __restrict__ rpairs, const i64* __restrict__ roff, i64 j0,
+                i64 j1, double2* __restrict__ psi) {
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
     double2* sm = reinterpret_cast<double2*>(smem_cell);  // [Da][CC]
@@ -261,24 +260,22 @@ k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, con
         const u32 r = i / CC, c = i - r * CC;
         if (c < ncol) sm[i] = psi[(i64)r * Db + c0 + c];
     }
-    const u64 mask_a = (u64(1) << n_orb) - 1;
     for (i64 j = j0; j < j1;) {
         __syncthreads();
         const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
         __syncthreads();
         for (int g = 0; g < n; ++g) {
-            const u32 xa = (u32)(G.x[g] & mask_a);
-            const u32 pxa = (u32)__popc(xa);
+            // owner (row, partner row) pairs of the generator were listed at plan time: one work item per (pair, column)
             const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
-            for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
-                const u32 r = i / CC, c = i - r * CC;
+            const i64 p0 = roff[j + g];
+            const u32 np = (u32)(roff[j + g + 1] - p0);
+            for (u32 i = threadIdx.x; i < np * CC; i += blockDim.x) {
+                const u32 q = i / CC, c = i - q * CC;
                 if (c >= ncol) continue;
-                const u32 ta = A.str[r];
-                if (2u * (u32)__popc(ta & xa) != pxa) continue;
-                const u32 ur = spin_rank(A, ta ^ xa);
-                if (ur <= r) continue;  // x_a != 0: the pair belongs to its smaller row
-                const u32 tb = B.str[c0 + c];
-                rotate_smem(sm[i], sm[ur * CC + c], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)), G.th[g], G.sc[g]);
+                const uint2 rp = __ldg(rpairs + p0 + q);
+                const u32 ta = A.str[rp.x], tb = B.str[c0 + c];
+                rotate_smem(sm[rp.x * CC + c], sm[rp.y * CC + c], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)),
+                            G.th[g], G.sc[g]);
             }
             __syncthreads();
         }
@@ -386,7 +383,28 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 }
                 RR->off[j + 1] = (i64)pairs.size();
             }
+            // column pairs per generator (independent of the row): valid columns and their partners; for x_a = 0 the
+            // pair lives in one row and is listed once (smaller column first)
+            std::vector<uint2> cpairs;
+            RR->coff.assign(n_rot + 1, 0);
+            if ((double)n_rot * (double)s->Db <= 5e8) {
+                for (i64 j = 0; j < n_rot; ++j) {
+                    const u64 xa = gen->h_xg[j] & mask_a, xb = gen->h_xg[j] >> s->n_orb;
+                    const int pxb = __builtin_popcountll(xb);
+                    for (i64 c = 0; c < s->Db; ++c) {
+                        const u64 tb = s->h_sb[c];
+                        if (2 * __builtin_popcountll(tb & xb) != pxb) continue;
+                        const i64 uc = xb ? (i64)(std::lower_bound(s->h_sb.begin(), s->h_sb.end(), tb ^ xb) - s->h_sb.begin()) : c;
+                        if (xa == 0 && uc <= c) continue;
+                        cpairs.push_back(make_uint2((u32)c, (u32)uc));
+                    }
+                    RR->coff[j + 1] = (i64)cpairs.size();
+                }
+            }
             cudaError_t e = RR->d_pairs.upload(pairs, st);
+            if (e == cudaSuccess) e = RR->d_cpairs.upload(cpairs, st);
+            if (e == cudaSuccess) e = RR->d_off.upload(RR->off, st);
+            if (e == cudaSuccess) e = RR->d_coff.upload(RR->coff, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             if (e != cudaSuccess) {
                 delete RR;
@@ -419,7 +437,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                                                 thetas[j], sc1, psi);
         BS_COUNT_LAUNCH(1);
     };
-    const bool batching = RR && !getenv("BS_ROT_PER_LAUNCH");
+    const bool batching = RR && RR->coff.back() > 0 && !getenv("BS_ROT_PER_LAUNCH");
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
         const u64 mask_a = (u64(1) << s->n_orb) - 1;
@@ -459,11 +477,11 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                     if (R == 2) {
                         BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                         k_rot_cell_rows<2><<<(unsigned)n_cells, 512, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
-                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_cpairs.p, RR->d_coff.p, j, e, psi);
                     } else {
                         BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                         k_rot_cell_rows<1><<<(unsigned)n_cells, 256, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
-                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_cpairs.p, RR->d_coff.p, j, e, psi);
                     }
                     BS_COUNT_LAUNCH(1);
                     launched = true;
@@ -478,11 +496,11 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                     if (CC == 8) {
                         BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                         k_rot_cell_cols<8><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
-                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_pairs.p, RR->d_off.p, j, e, psi);
                     } else {
                         BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                         k_rot_cell_cols<2><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
-                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_pairs.p, RR->d_off.p, j, e, psi);
                     }
                     BS_COUNT_LAUNCH(1);
                     launched = true;
