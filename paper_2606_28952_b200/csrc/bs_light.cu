@@ -146,11 +146,12 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
         __syncthreads();
         const uint4* __restrict__ items4 = reinterpret_cast<const uint4*>(P.items);
         const u32 nk0 = reinterpret_cast<const u32*>(P.xa_hdr)[3] - L.key0;  // keys of the x_a = 0 header (header 0)
+        const u32 wid = tid >> 5;
+        const bool alpha_first = L.order == 1 ? (wid & 1u) : L.order == 2 ? (wid >= kLT / 64) : L.order == 3 ? ((wid >> 2) & 1u) : false;
         u32 it_n = 0;
         for (i64 r = r0; r < r1; r += rs, ++it_n) {
             const u32 b = it_n & 1u;
             if (tid == 0 && r + rs < r1) stage(r + rs, b ^ 1u);  // buffer b^1 was released by the barrier ending the previous row
-            mbar_wait(bar + b, (it_n >> 1) & 1u);
             const double2* __restrict__ srow = rowbuf + (size_t)b * (Db + 1);
             const double* __restrict__ Vr = L.vtab + __ldg(L.voff + r);
             double2 acc[kLC];
@@ -161,8 +162,11 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
                 for (int k = 0; k < kLC; ++k)
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(ep.acc + r * (i64)Db + col[k]));
             }
+            if (L.lut_nq && r + rs < r1) build_lut(r + rs, b ^ 1u);  // visible after the barrier that ends this row
+            // shared-memory phase: diagonal and beta hops from the staged row
+            auto smem_phase = [&]() {
+            mbar_wait(bar + b, (it_n >> 1) & 1u);
             if (L.lut_nq) {
-                if (r + rs < r1) build_lut(r + rs, b ^ 1u);  // visible after the barrier that ends this row
                 const double* __restrict__ lut = slut + b * 128;
                 const double f0 = __ldg(Vr + (d_key0 - L.key0));
 #pragma unroll
@@ -220,7 +224,9 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
                     }
                 }
             }
-            // alpha hops: row axpys from global memory (coalesced 128-bit loads), two entries in flight
+            };
+            // global phase: alpha hops are row axpys from global memory / L2 (coalesced 128-bit loads), two entries in flight
+            auto alpha_phase = [&]() {
             const i64 e0 = __ldg(P.row_off + r), e1 = __ldg(P.row_off + r + 1);
             i64 e = e0 + 1;
             for (; e + 1 < e1; e += 2) {
@@ -253,6 +259,16 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
                     acc[k].x += f0 * a[k].x;
                     acc[k].y += f0 * a[k].y;
                 }
+            }
+            };
+            // Half of the warps run the global phase first: all warps leave the row barrier together, so without this
+            // the shared-memory pipe idles while every warp waits on L2 and vice versa.
+            if (alpha_first) {
+                alpha_phase();
+                smem_phase();
+            } else {
+                smem_phase();
+                alpha_phase();
             }
 #pragma unroll
             for (int k = 0; k < kLC; ++k) {
@@ -348,6 +364,8 @@ int bs_light_apply(bs_rowplan* R, const double2* psi, double2* out, i64 lo, i64 
     L.item_split = h0.item_split;
     L.key0 = h0.key0;
     L.key_split = h0.key_split;
+    L.order = 3;
+    if (const char* o = getenv("BS_LIGHT_ORDER")) L.order = atoi(o);  // tuning: 0 = every warp runs the shared-memory phase first
     L.lut_nq = 0;
     if (h0.item_split - h0.item0 == 1) {
         const u32 nk = R->h_items[h0.item0].nkeys;
