@@ -373,7 +373,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {"q28_hubbard": 9.26e8}   # profiles/r01_v3_q28_k_light_full.md, fused apply+axpy launch
+TRAFFIC_NCU = {"q28_hubbard": 9.22e8}   # profiles/r01_v4_q28_k_light_full.md, fused apply+axpy launch
 
 
 def run_reference(args):
