@@ -29,18 +29,25 @@ __device__ __forceinline__ u32 light_slot(u32 col) { return (col % kLT) * kLC + 
 
 // list build: entry j of a column = j-th valid listed table (source column | sign << 15), padded with D_beta
 // (the zero amplitude kept behind each staged row)
-__global__ void k_light_list(SpinTab B, const uint2* __restrict__ tkeys, int n_listed, int l_max,
+__global__ void k_light_list(SpinTab B, const uint2* __restrict__ tkeys, int n_listed, int l_max, int allow_by_table,
                              unsigned short* __restrict__ L, int* __restrict__ cnt) {
     const u32 col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (u32)kLW) return;
     const u32 slot = light_slot(col);
+    // When some column uses every listed table (l_max == n_listed: the Hubbard chain) compaction saves nothing, and
+    // slot t = table t keeps the lanes of a warp on the same hop: neighbouring targets then read neighbouring sources
+    // (fewer shared-memory bank conflicts than the compacted order, which mixes hops across lanes).
+    const bool by_table = allow_by_table && l_max == n_listed;
     int j = 0;
     if (col < B.D) {
         const u32 tb = B.str[col];
         for (int t = 0; t < n_listed; ++t) {
             const uint2 k = tkeys[t];
-            if (2 * __popc(tb & k.x) != __popc(k.x)) continue;
-            if (l_max) L[(i64)j * kLW + slot] = (unsigned short)(spin_rank(B, tb ^ k.x) | ((u32)(__popc(tb & k.y) & 1) << 15));
+            const bool valid = 2 * __popc(tb & k.x) == __popc(k.x);
+            if (!valid && !(l_max && by_table)) continue;
+            if (l_max)
+                L[(i64)j * kLW + slot] =
+                    valid ? (unsigned short)(spin_rank(B, tb ^ k.x) | ((u32)(__popc(tb & k.y) & 1) << 15)) : (unsigned short)B.D;
             ++j;
         }
     }
@@ -311,7 +318,7 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
         std::vector<uint2> tk(R->h_tkeys.begin(), R->h_tkeys.begin() + n_listed);
         BS_CUDA(d_tk.upload(tk, st));
         BS_CUDA(d_cnt.alloc(kLW));
-        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, 0, nullptr, d_cnt.p);
+        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, 0, 0, nullptr, d_cnt.p);
         std::vector<int> hc(kLW);
         BS_CUDA(cudaMemcpyAsync(hc.data(), d_cnt.p, kLW * 4, cudaMemcpyDeviceToHost, st));
         BS_CUDA(cudaStreamSynchronize(st));
@@ -321,7 +328,8 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
     if (smem > 227 * 1024 - 1024) return BS_OK;
     BS_CUDA(R->d_llist.alloc((size_t)std::max(1, l_max) * kLW));
     if (l_max > 0) {
-        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, l_max, R->d_llist.p, d_cnt.p);
+        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, l_max, getenv("BS_LIGHT_COMPACT") ? 0 : 1, R->d_llist.p,
+                                                d_cnt.p);
         BS_COUNT_LAUNCH(2);
     }
     // V table
