@@ -328,9 +328,12 @@ def run_ours(args):
     applies_per_step = TAYLOR_ORDER + 1
     if rank == 0:
         value = world * applies_per_step * args.steps / (total_ms * 1e-3)
-        # dominant kernel: k_rows (Taylor launches). Algorithmic bytes per Taylor step:
-        # k=1: 32 D; k=2..order-1: 64 D (in, out, acc r+w); k=order: 48 D; + tables each launch.
-        bytes_taylor = (32 + 64 * (TAYLOR_ORDER - 2) + 48) * D + TAYLOR_ORDER * tb
+        # dominant kernel: the apply kernel of the Taylor launches. Algorithmic bytes per Taylor step (bs_taylor_step
+        # accumulates terms in pairs): odd k: 32 D (in, out); even k: 64 D (in, out, acc r+w); the last launch writes no
+        # out (48 D even, 48 D odd: in + acc r+w); + tables each launch.  Order 12: (6*32 + 5*64 + 48) D = 560 D.
+        per_launch = [(32 if k % 2 else 64) for k in range(1, TAYLOR_ORDER + 1)]
+        per_launch[-1] = 48
+        bytes_taylor = sum(per_launch) * D + TAYLOR_ORDER * tb
         launch_ms = taylor_ms / (args.steps * TAYLOR_ORDER)
         achieved = bytes_taylor / TAYLOR_ORDER / launch_ms / 1e6
         line = {

@@ -32,6 +32,7 @@ ref8 = orc.hubbard_h(8, 1.0, 4.0)
 cases.append(('hub8', ref8, jw.hubbard_raw_terms(8, 1.0, 4.0), 8, 4, 3))
 ref10 = orc.hubbard_h(10, 1.0, 4.0)
 cases.append(('hub10', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 4))     # light path (D_beta = 210 >= 64)
+cases.append(('hub10h', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 5))    # light path, list slots by table (l_max = 9 bonds)
 h, g = si.integrals(7, 77)
 cases.append(('mol7', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 7, 2, 5))
 # generic complex operator (multi-key, POPC signs, complex weights)
@@ -48,7 +49,7 @@ for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2)]
     sec, osec = bs.bs_sector_build(n, na, nb), orc.Sector(n, na, nb)
     desc = bs.bs_plan_describe(op, sec)
     assert want_kernel in desc, (want_kernel, desc)
-    if name == 'hub10' and want_kernel == 'rows_v2':
+    if name in ('hub10', 'hub10h') and want_kernel == 'rows_v2':
         assert ('+light' in desc) == (os.environ.get('BS_NO_LIGHT') is None), desc
     psi = si.random_state(osec.dim, 5)
     want = osec.apply_grouped(ref, psi) if osec.dim > 100000 else osec.apply(ref, psi)
@@ -76,6 +77,8 @@ print('PATH OK')
 @pytest.mark.parametrize("env,kernel", [
     ({}, "rows_v2"),
     ({"BS_NO_LIGHT": "1"}, "rows_v2"),
+    ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0"}, "rows_v2"),   # light kernel: compacted list, one phase order
+    ({"BS_LIGHT_ORDER": "1"}, "rows_v2"),
     ({"BS_KERNEL": "v1"}, "sector_v1"),
     ({"BS_KERNEL": "v2inrow"}, "kernel="),      # q24's beta-only groups do not fit in-row: falls back to v1 there
     ({"BS_ROW_WIN": "24"}, "n_win="),
