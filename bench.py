@@ -7,7 +7,7 @@
 Headline workload (config.workload): BASELINE.json configs[2], the 28-qubit Fermi-Hubbard chain
 (sector dim 11,778,624; 188.5 MB per vector, larger than the 126 MB L2, so no L2 flush is needed).
 A "step" is one pass of the hot path over one state vector: one order-12 shifted Taylor step of
-exp(-i H dt) (a7: 12 fused apply+axpy launches of the a4 kernel) followed by one fused energy
+exp(-i H dt) (a7: 12 fused apply+axpby launches of the a4 kernel, terms accumulated in pairs) followed by one fused energy
 (a5: bs_expect) = 13 H applications.  a1-a3 (grouping, sector tables) are built once per operator and
 reported as setup_ms; a6 (rotations) is timed in the q24 entry of `per_config`.
 value = H applications per second over all ranks (each rank propagates its own state: weak scaling,
@@ -355,7 +355,7 @@ def run_ours(args):
                     "h2d_bytes_per_step": 16 * D, "d2h_bytes_per_step": 16 * D + 16, "steps": e2e_steps,
                     "pipeline": "H2D of step i+1 and D2H of step i-1 overlap step i (2 device buffers, 3 streams)"},
             "roofline": {"bound": "hbm", "kernel": ("k_light<0>" if "+light" in bs.bs_plan_describe(op, sec) else "k_rows<MODE_FINAL>")
-                         + " (fused apply+axpy launches of bs_taylor_step)",
+                         + " (the 12 apply+axpby launches of bs_taylor_step)",
                          "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
                          "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
                          "launch_ms": launch_ms, "traffic": TRAFFIC_NCU.get(name)},
@@ -376,7 +376,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {"q28_hubbard": 9.22e8}   # profiles/r01_v4_q28_k_light_full.md, fused apply+axpy launch
+TRAFFIC_NCU = {"q28_hubbard": 7.14e8}   # profiles/r01_v6_q28_k_light_full.md: mean of an odd (506 MB) and an even (922 MB) Taylor launch
 
 
 def run_reference(args):
