@@ -376,7 +376,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {"q28_hubbard": 7.14e8}   # profiles/r01_v6_q28_k_light_full.md: mean of an odd (506 MB) and an even (922 MB) Taylor launch
+TRAFFIC_NCU = {"q28_hubbard": 6.90e8}   # profiles/r01_v6_q28_k_light_full.md: mean of an odd (490 MB) and an even (890 MB) Taylor launch
 
 
 def run_reference(args):

@@ -39,7 +39,9 @@ __device__ __forceinline__ double2 block_sum(double2 v, double2* sh) {
     return v;
 }
 
-template <bool EXPECT>
+// STREAM: out / acc are touched once per launch: streaming (evict-first) accesses leave L2 to the state vector
+// whose rows are re-read as hop sources
+template <bool EXPECT, bool STREAM = false>
 __device__ __forceinline__ void finish_target(double2 a, double2 pin, i64 idx, double2* __restrict__ out,
                                               const Epilogue& ep, double2& dot) {
     if (EXPECT) {
@@ -53,7 +55,7 @@ __device__ __forceinline__ void finish_target(double2 a, double2 pin, i64 idx, d
         r.x += b.x;
         r.y += b.y;
         if (ep.acc) {
-            double2 c = ep.acc[idx];
+            double2 c = STREAM ? __ldcs(ep.acc + idx) : ep.acc[idx];
             c.x += r.x;
             c.y += r.y;
             if (ep.add_in) {
@@ -61,11 +63,16 @@ __device__ __forceinline__ void finish_target(double2 a, double2 pin, i64 idx, d
                 c.y += pin.y;
             }
             if (ep.scale_acc) c = cmul(ep.scale, c);
-            ep.acc[idx] = c;
+            if (STREAM) __stcs(ep.acc + idx, c);
+            else ep.acc[idx] = c;
         }
-        if (ep.store_out) out[idx] = r;
+        if (ep.store_out) {
+            if (STREAM) __stcs(out + idx, r);
+            else out[idx] = r;
+        }
     } else {
-        out[idx] = a;
+        if (STREAM) __stcs(out + idx, a);
+        else out[idx] = a;
     }
 }
 

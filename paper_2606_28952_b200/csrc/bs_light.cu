@@ -281,7 +281,8 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
             for (int k = 0; k < kLC; ++k) {
                 if (!ok[k]) continue;
                 const i64 idx = r * (i64)Db + col[k];
-                finish_target<MODE == 2>(acc[k], srow[col[k]], idx, out, ep, dot);
+                if (L.stream) finish_target<MODE == 2, true>(acc[k], srow[col[k]], idx, out, ep, dot);
+                else finish_target<MODE == 2, false>(acc[k], srow[col[k]], idx, out, ep, dot);
             }
             __syncthreads();  // everyone is done with buffer b before row r + 2 is staged into it
         }
@@ -372,6 +373,7 @@ int bs_light_apply(bs_rowplan* R, const double2* psi, double2* out, i64 lo, i64 
     L.item_split = h0.item_split;
     L.key0 = h0.key0;
     L.key_split = h0.key_split;
+    L.stream = getenv("BS_LIGHT_STREAM") ? atoi(getenv("BS_LIGHT_STREAM")) : 1;
     L.order = 3;
     if (const char* o = getenv("BS_LIGHT_ORDER")) L.order = atoi(o);  // tuning: 0 = every warp runs the shared-memory phase first
     L.lut_nq = 0;

@@ -102,6 +102,7 @@ struct LightDev {
     int l_max;
     u32 item0, item_split, key0, key_split;  // of the x_a = 0 header
     int lut_nq;                              // nibble tables of the diagonal (0: generic key loop)
+    int stream;                              // streaming (evict-first) stores of out / acc
     int order;                               // which warps run the alpha-hop (global) phase before the shared-memory phase
 };
 int bs_light_build(bs_rowplan* R, cudaStream_t st);
