@@ -267,6 +267,26 @@ def test_taylor_step_small_hubbard(bs, orc):
     assert abs(bs.bs_vdot(sec, d, d).real - 1.0) <= 1e-12
 
 
+@pytest.mark.parametrize("order", [2, 3, 4, 7, 12, 13])
+def test_taylor_step_orders(bs, orc, order):
+    """bs_taylor_step accumulates the terms in pairs (even launches add input + output): even and odd orders, the
+    shortest ones included, on the light-kernel path (10 sites, 5 + 5) against the oracle's Eq. 6-7 loop."""
+    import torch
+    from paper_2606_28952_b200 import jw_terms as jw
+    L = 10
+    ref = orc.hubbard_h(L, 1.0, 4.0)
+    op = bs.bs_group_xmask(*jw.hubbard_raw_terms(L, 1.0, 4.0), 2 * L, 1e-12)
+    osec, sec = orc.Sector(L, 5, 5), bs.bs_sector_build(L, 5, 5)
+    psi = si.random_state(osec.dim, 14)
+    d = to_device(psi)
+    work = torch.empty(2 * sec.dim, dtype=torch.complex128, device="cuda")
+    e0 = bs.bs_expect(op, sec, d).real
+    for _ in range(2):
+        bs.bs_taylor_step(op, sec, d, work, 0.03, order, e0)
+        osec.taylor_step(ref, psi, 0.03, order, e0)
+    assert rel_l2(to_host(d), psi) <= TOL_L2
+
+
 def test_q28_hubbard_single_apply(bs, orc):
     """Config 3 operator at full size: one apply vs the definition-mode oracle (95 terms x 1.2e7)."""
     cfg = si.CONFIGS["q28_hubbard"]
