@@ -170,11 +170,10 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
 template <bool REALW, int CPT, bool WINDOWED, bool UNIF>
 __device__ __forceinline__ void list_pass(const RowPlanDev& P, const typename VT<REALW>::type* __restrict__ sVx,
                                           typename VT<REALW>::type vu, const double2* __restrict__ srow, u32 w0, u32 wn,
-                                          u32 tpos, double2 (&acc)[CPT]) {
+                                          u32 tpos, double2 (&acc)[CPT], int slot0, int l_max) {
     using V = VT<REALW>;
-    const u32* __restrict__ p = P.ltab + tpos;
     const u32 stride = (u32)P.tstride;
-    const int l_max = P.l_max;
+    const u32* __restrict__ p = P.ltab + (size_t)slot0 * stride + tpos;
     u32 en[CPT], n1[CPT];
     auto load = [&](u32 (&e)[CPT]) {
         if (CPT == 4) {
@@ -327,14 +326,21 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                         process_entry<REALW, CPT, true, false>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, 0u, wn,
                                                                tpos, col, tb, acc);
                     if (listed) {
-                        if (unif) list_pass<REALW, CPT, false, true>(P, sVx, vbase[hs.w - h4.z], srow, 0u, wn, tpos, acc);
-                        else list_pass<REALW, CPT, false, false>(P, sVx, V::zero(), srow, 0u, wn, tpos, acc);
+                        if (unif) list_pass<REALW, CPT, false, true>(P, sVx, vbase[hs.w - h4.z], srow, 0u, wn, tpos, acc, 0, P.l_max);
+                        else list_pass<REALW, CPT, false, false>(P, sVx, V::zero(), srow, 0u, wn, tpos, acc, 0, P.l_max);
                     }
                 } else {
                     if (h4.x < hs.z)
                         process_entry<REALW, CPT, true, true>(P, items4, h4.x, hs.z, h4.z, vbase, srow, srcp, w0, wn,
                                                               tpos, col, tb, acc);
-                    if (listed) list_pass<REALW, CPT, true, false>(P, sVx, V::zero(), srow, w0, wn, tpos, acc);
+                    if (listed) {
+                        if (P.l_woff) {  // this window's own list: no window test, padding hits the zero amplitude
+                            const int s0 = __ldg(P.l_woff + w);
+                            const int ns = __ldg(P.l_woff + P.n_win + 1 + w * P.l_nchunks + (int)chunk);
+                            if (ns > 0) list_pass<REALW, CPT, false, false>(P, sVx, V::zero(), srow, w0, wn, tpos, acc, s0, ns);
+                        } else
+                            list_pass<REALW, CPT, true, false>(P, sVx, V::zero(), srow, w0, wn, tpos, acc, 0, P.l_max);
+                    }
                 }
             }
         }

@@ -32,14 +32,15 @@ __global__ void k_fill_ttab(SpinTab B, const uint2* __restrict__ keys, i64 tstri
 }
 
 // l_max == 0: count the valid listed tables of every slot; else write the padded list
+// Only entries whose source column lies in [w0, w0 + wn) are taken (one list per source-row window).
 __global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, int n_listed, int l_max, u32 pad_src,
-                             u32* __restrict__ L, int* __restrict__ cnt) {
+                             u32 w0, u32 wn, u32* __restrict__ L, int* __restrict__ cnt) {
     const i64 slot = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (slot >= tstride) return;
     int j = 0;
     for (int t = 0; t < n_listed; ++t) {
         const u32 e = T[(i64)t * tstride + slot];
-        if (e == 0xFFFFu) continue;
+        if (e == 0xFFFFu || ((e & 0x7FFFu) - w0) >= wn) continue;
         if (l_max) L[(i64)j * tstride + slot] = e | ((u32)t << 16);
         ++j;
     }
@@ -272,14 +273,44 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
         DevBuf<int> lcnt;
         BS_CUDA(lcnt.alloc(R->tstride));
         const unsigned lb = (unsigned)((R->tstride + 255) / 256);
-        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, 0, 0u, nullptr, lcnt.p);
         std::vector<int> hl(R->tstride);
-        BS_CUDA(cudaMemcpyAsync(hl.data(), lcnt.p, R->tstride * 4, cudaMemcpyDeviceToHost, st));
-        BS_CUDA(cudaStreamSynchronize(st));
-        for (int v : hl) R->l_max = std::max(R->l_max, v);
-        BS_CUDA(R->d_ltab.alloc((size_t)std::max(1, R->l_max) * R->tstride));
-        k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, R->l_max, (u32)Db, R->d_ltab.p, lcnt.p);
-        BS_COUNT_LAUNCH(2);
+        // With windowed source rows every window gets its own list (only the entries whose source lies in it), so a
+        // window pass walks its own entries instead of the whole list with a window test per entry. Padding entries
+        // point at the zero amplitude behind the staged window (column w0 + win_cols: must fit the 15-bit source field).
+        const bool split = n_win > 1 && (i64)n_win * win <= 32767 && !getenv("BS_ROW_NO_SPLIT");
+        const int n_lists = split ? n_win : 1;
+        std::vector<int> woff(n_lists + 1, 0), wcnt;
+        for (int w = 0; w < n_lists; ++w) {
+            const u32 w0 = split ? (u32)(w * win) : 0u, wn = split ? (u32)win : 0xFFFFFFFFu;
+            k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, 0, 0u, w0, wn, nullptr, lcnt.p);
+            BS_CUDA(cudaMemcpyAsync(hl.data(), lcnt.p, R->tstride * 4, cudaMemcpyDeviceToHost, st));
+            BS_CUDA(cudaStreamSynchronize(st));
+            int m = 0;
+            for (int v : hl) m = std::max(m, v);
+            // slots a block of column chunk c has to walk in this window: the longest list among its own columns
+            const i64 per_chunk = (i64)R->threads * R->cpt;
+            for (int c = 0; c < R->n_chunks; ++c) {
+                int mc = 0;
+                for (i64 sl = c * per_chunk; sl < (c + 1) * per_chunk; ++sl) mc = std::max(mc, hl[sl]);
+                wcnt.push_back(mc);
+            }
+            woff[w + 1] = woff[w] + m;
+            R->l_max = std::max(R->l_max, m);
+        }
+        BS_CUDA(R->d_ltab.alloc((size_t)std::max(1, woff[n_lists]) * R->tstride));
+        for (int w = 0; w < n_lists; ++w) {
+            const int m = woff[w + 1] - woff[w];
+            if (m == 0) continue;
+            const u32 w0 = split ? (u32)(w * win) : 0u, wn = split ? (u32)win : 0xFFFFFFFFu;
+            k_list_build<<<lb, 256, 0, st>>>(R->d_ttab.p, R->tstride, n_listed, m, split ? w0 + (u32)win : (u32)Db, w0, wn,
+                                             R->d_ltab.p + (size_t)woff[w] * R->tstride, lcnt.p);
+        }
+        BS_COUNT_LAUNCH(2 * n_lists);
+        if (split) {  // [window offsets (n_win + 1)][slots per (window, chunk)]
+            woff.insert(woff.end(), wcnt.begin(), wcnt.end());
+            BS_CUDA(R->d_lwoff.upload(woff, st));
+        }
+        R->l_split = split;
     }
     // per-row valid alpha masks
     DevBuf<int> cnt;
@@ -319,6 +350,8 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     d.chunk_cols = R->chunk_cols;
     d.ltab = R->d_ltab.p;
     d.l_max = R->l_max;
+    d.l_woff = R->l_split ? R->d_lwoff.p : nullptr;
+    d.l_nchunks = R->n_chunks;
     d.n_listed = n_listed;
     return BS_OK;
 }

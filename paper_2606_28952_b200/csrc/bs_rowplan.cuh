@@ -53,7 +53,9 @@ struct RowPlanDev {
     int chunk_cols;             // target columns per thread block
     // Column list (compaction of the listed column tables over table ids): entry j of slot s is
     // source column | sign << 15 | table id << 16; padded with (0, 0, n_listed) whose V slot is always 0.
-    const u32* ltab;            // [l_max][tstride]
+    const u32* ltab;            // [l_max][tstride]; with l_woff: window w owns list slots [l_woff[w], l_woff[w + 1])
+    const int* l_woff;          // nullptr: one list for all windows (entries carry a window test); then per (window, chunk) slot counts
+    int l_nchunks;
     int l_max, n_listed;
 };
 
@@ -69,6 +71,8 @@ struct bs_rowplan {
     DevBuf<double2> d_s_w;
     DevBuf<unsigned short> d_ttab;
     DevBuf<u32> d_ltab;
+    DevBuf<int> d_lwoff;
+    bool l_split = false;
     int l_max = 0, n_listed = 0;
     DevBuf<i64> d_row_off;
     DevBuf<uint4> d_row_ent;

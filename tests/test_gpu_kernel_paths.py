@@ -81,7 +81,8 @@ print('PATH OK')
     ({"BS_LIGHT_ORDER": "1"}, "rows_v2"),
     ({"BS_KERNEL": "v1"}, "sector_v1"),
     ({"BS_KERNEL": "v2inrow"}, "kernel="),      # q24's beta-only groups do not fit in-row: falls back to v1 there
-    ({"BS_ROW_WIN": "24"}, "n_win="),
+    ({"BS_ROW_WIN": "24"}, "n_win="),                                  # windowed rows, one column list per window
+    ({"BS_ROW_WIN": "24", "BS_ROW_NO_SPLIT": "1"}, "n_win="),          # windowed rows, one list with a window test
     ({"BS_ROW_WIN": "24", "BS_KERNEL": "v2inrow"}, "kernel="),
 ])
 def test_kernel_path(env, kernel):
