@@ -21,6 +21,7 @@
 //   orc_taylor_step ...... high-order sub-stepped series at 6 sites; reversibility (P11)
 //   orc_apply_grouped .... equals orc_apply_terms (P12)
 //   orc_apply_sampled .... equals orc_apply_terms on the sampled targets
+//   orc_apply_grouped_slab  equals orc_apply_terms on every row slab (P12)
 #include <algorithm>
 #include <cmath>
 #include <complex>
@@ -40,6 +41,9 @@ using i64 = int64_t;
 namespace {
 
 inline int popc(u64 v) { return __builtin_popcountll(v); }
+// popcnt(v) mod 2 of a 32-bit word by xor-folding (each fold halves the width and keeps the parity); written
+// without the popcount builtin so that the compiler can vectorise loops over it (orc_apply_grouped_slab)
+inline uint32_t parity32(uint32_t v) { v ^= v >> 16; v ^= v >> 8; v ^= v >> 4; v ^= v >> 2; v ^= v >> 1; return v & 1u; }
 
 // ---------------------------------------------------------------------------------------
 // Pauli strings in XZ-ordered form R(X,Z) = (x)_k sx^{a_k} sz^{b_k}  (Eq. 13)
@@ -423,6 +427,79 @@ void orc_apply_grouped(void* s, const u64* x, const u64* z, const double* c_reim
                 for (i64 k = offs[g]; k < offs[g + 1]; ++k) ph += (popc(z[k] & src) & 1) ? -C[k] : C[k];
                 orow[j] += ph * psi[ia * S->Db + ib];
             }
+        }
+    }
+}
+
+// The same Eq. 27 gather for an alpha-row slab [row_lo, row_hi), written to a slab-sized buffer
+// out_slab[(i - row_lo) * D_b + j], with the beta-string search of Eq. 28 ("two
+// smaller spin-string index searches") done ONCE per distinct beta mask instead of once per
+// (row, group, column): whether s_b[j] ^ x_b is a sector string, and where it sits, does not depend
+// on the row.  Same loops and same arithmetic as orc_apply_grouped otherwise.  Used to write the
+// full-size goldens of configs 4-5 (tests/golden/make_fullsize_golden.py), where the per-row search
+// makes orc_apply_grouped take days.  Pinned against orc_apply_terms (P12).  Sector mode only.
+void orc_apply_grouped_slab(void* s, const u64* x, const u64* z, const double* c_reim, i64 M,
+                            const double* psi_reim, double* out_slab_reim, i64 row_lo, i64 row_hi) {
+    Sector* S = (Sector*)s;
+    if (S->full) return;
+    const cd* psi = (const cd*)psi_reim;
+    cd* out = (cd*)out_slab_reim;
+    std::vector<i64> offs;
+    for (i64 k = 0; k < M; ++k)
+        if (k == 0 || x[k] != x[k - 1]) offs.push_back(k);
+    offs.push_back(M);
+    i64 G = (i64)offs.size() - 1;
+    std::vector<cd> C(M);  // C_k = c_k i^{ny_k} (Eq. 18)
+    for (i64 k = 0; k < M; ++k) C[k] = cd(c_reim[2 * k], c_reim[2 * k + 1]) * pow_i(popc(x[k] & z[k]));
+    // per distinct beta mask: the (target column j, source column ib, source string) triples with
+    // s_b[j] ^ x_b in the sector
+    struct BetaPairs { std::vector<int32_t> tj, ib; std::vector<uint32_t> src; };  // spin strings have n <= 32 bits
+    std::map<u64, BetaPairs> beta_pairs;
+    for (i64 g = 0; g < G; ++g) {
+        u64 xg = x[offs[g]];
+        if (S->n < 32 && (xg >> (2 * S->n))) continue;
+        u64 xb = xg >> S->n;
+        if (beta_pairs.count(xb)) continue;
+        BetaPairs& v = beta_pairs[xb];
+        for (i64 j = 0; j < S->Db; ++j) {
+            i64 ib = Sector::pos(S->sb, S->sb[j] ^ xb);
+            if (ib < 0) continue;
+            v.tj.push_back((int32_t)j); v.ib.push_back((int32_t)ib); v.src.push_back((uint32_t)S->sb[ib]);
+        }
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (i64 i = row_lo; i < row_hi; ++i) {
+        cd* orow = out + (i - row_lo) * S->Db;
+        for (i64 j = 0; j < S->Db; ++j) orow[j] = cd(0, 0);
+        std::vector<double> ph_re(S->Db), ph_im(S->Db);  // phase sum of the group, per valid target column
+        for (i64 g = 0; g < G; ++g) {
+            u64 xg = x[offs[g]];
+            if (S->n < 32 && (xg >> (2 * S->n))) continue;
+            u64 xa = xg & S->mask_a, xb = xg >> S->n;
+            u64 srca = S->sa[i] ^ xa;
+            i64 ia = Sector::pos(S->sa, srca);
+            if (ia < 0) continue;
+            const BetaPairs& bp = beta_pairs.find(xb)->second;
+            const i64 np = (i64)bp.tj.size();
+            for (i64 p = 0; p < np; ++p) { ph_re[p] = 0; ph_im[p] = 0; }
+            // Eq. 31 (reading U7): the sign (-1)^{popcnt(z & s)} of Eq. 27 splits into an alpha
+            // factor, the same for the whole row, and a beta factor: popcnt(z & s) = popcnt(z_a & s_a) + popcnt(z_b & s_b).
+            // Strings in the order given; for each string the loop runs over the valid columns.
+            for (i64 k = offs[g]; k < offs[g + 1]; ++k) {
+                double sa = (popc(z[k] & S->mask_a & srca) & 1) ? -1.0 : 1.0;
+                double cre = sa * C[k].real(), cim = sa * C[k].imag();
+                uint32_t zb = (uint32_t)(z[k] >> S->n);
+                const uint32_t* __restrict src = bp.src.data();
+                double* __restrict pre = ph_re.data();
+                double* __restrict pim = ph_im.data();
+                for (i64 p = 0; p < np; ++p) {
+                    double sb = 1.0 - 2.0 * (double)(int32_t)parity32(zb & src[p]);
+                    pre[p] += sb * cre;
+                    pim[p] += sb * cim;
+                }
+            }
+            const cd* prow = psi + ia * S->Db;
+            for (i64 p = 0; p < np; ++p) orow[bp.tj[p]] += cd(ph_re[p], ph_im[p]) * prow[bp.ib[p]];
         }
     }
 }

@@ -13,7 +13,9 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libbs_oracle.so")
+# BS_ORACLE_SO: use an oracle library built elsewhere from the same source (e.g. with -O3 -march=native for the
+# hours-long golden run of tests/golden/make_fullsize_golden.py); default: the portable in-tree -O2 build.
+_SO = os.environ.get("BS_ORACLE_SO") or os.path.join(_HERE, "libbs_oracle.so")
 _SRC = os.path.join(_HERE, "bs_oracle.cpp")
 _lib = None
 
@@ -25,6 +27,8 @@ _f64p = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
 
 def build(force: bool = False) -> str:
     """Compile the oracle with g++ (plain C++17 + OpenMP).  Building is not using."""
+    if os.environ.get("BS_ORACLE_SO"):
+        return _SO
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
         cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC]
         subprocess.check_call(cmd)
@@ -62,6 +66,8 @@ def lib():
                                         C.c_int64, _f64p]
         L.orc_apply_grouped.argtypes = [C.c_void_p, _u64p, _u64p, _f64p, C.c_int64, _f64p, _f64p,
                                         C.c_int64, C.c_int64]
+        L.orc_apply_grouped_slab.argtypes = [C.c_void_p, _u64p, _u64p, _f64p, C.c_int64, _f64p, _f64p,
+                                             C.c_int64, C.c_int64]
         L.orc_vdot.argtypes = [_f64p, _f64p, C.c_int64, _f64p]
         L.orc_rot_fermionic.argtypes = [C.c_void_p, _i32p, C.c_int, _i32p, C.c_int, C.c_double, _f64p]
         L.orc_taylor_step.argtypes = [C.c_void_p, _u64p, _u64p, _f64p, C.c_int64, C.c_double,
@@ -188,6 +194,14 @@ class Sector:
             row_hi = self.dim if self.n_alpha < 0 else self.dim_alpha
         lib().orc_apply_grouped(self._h, op.x, op.z, _reim(op.c), len(op), _reim(psi), _reim(out),
                                 row_lo, row_hi)
+        return out
+
+    def apply_grouped_slab(self, op: PauliOp, psi, row_lo, row_hi):
+        """Rows [row_lo, row_hi) of H psi as a (row_hi - row_lo, dim_beta) array (beta search hoisted)."""
+        psi = np.ascontiguousarray(psi, np.complex128)
+        out = np.empty((row_hi - row_lo, self.dim_beta), np.complex128)
+        lib().orc_apply_grouped_slab(self._h, op.x, op.z, _reim(op.c), len(op), _reim(psi), _reim(out),
+                                     row_lo, row_hi)
         return out
 
     def rot_fermionic(self, psi, cre, ann, theta):

@@ -148,9 +148,10 @@ def test_p3_config_counts_match_survey_table():
 
 
 # ---------------------------------------------------------------- P4 dense Kronecker vs fermionic
-@pytest.mark.parametrize("n", [2, 3])
+@pytest.mark.parametrize("n", [2, 3, 6])
 def test_p4_molecular_dense_equals_fermionic_matrix(n):
-    h, g = S.integrals(n, 77 + n)
+    # n = 6 is config 1 itself (12 qubits, the survey's "<= 12 qubits"): 4096 x 4096, sparse on both sides
+    h, g = S.integrals(n, 1001 if n == 6 else 77 + n)
     op = O.molecular_h(h, g)
     nq = 2 * n
     Hp = R.pauli_sum_matrix(op.x, op.z, op.c, nq).toarray()
@@ -472,3 +473,9 @@ def test_p12_grouped_and_sampled_equal_definition(kind):
         slab = sec.apply_grouped(op, psi, 1, 3)
         db = sec.dim_beta
         assert np.array_equal(slab[db:3 * db], fast[db:3 * db]) and not slab[:db].any() and not slab[3 * db:].any()
+        # slab mode with the beta search hoisted (the writer of the full-size goldens): every slab vs the definition
+        da = sec.dim_alpha
+        for lo, hi in ((0, da), (0, 1), (1, 3), (da - 2, da)):
+            got = sec.apply_grouped_slab(op, psi, lo, hi).reshape(-1)
+            want = ref[lo * db:hi * db]
+            assert np.linalg.norm(got - want) <= 1e-13 * max(1.0, np.linalg.norm(ref))
