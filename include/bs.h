@@ -60,7 +60,8 @@ typedef enum {
 /* ---- a1 + a2: canonical reduction and X-mask grouping (Eq. 24).
  * x, z [host] u64[M]; coeff_reim [host] double[2M] (true-Pauli coefficients c_k).
  * mode BS_MODE_CANONICAL: sort by key (x major, z minor, unsigned ascending; stable), sum the
- *   coefficients of equal keys in INPUT order, drop |c| < eps_drop, segment by x.  Runs on the
+ *   coefficients of equal keys in INPUT order, drop |c| < eps_drop (and, also with eps_drop = 0, merged
+ *   coefficients that are exactly zero), segment by x.  Runs on the
  *   device (radix sort, segmented sum, compaction).  seq_offsets must be NULL.
  * mode BS_MODE_SEQUENCE: strings [seq_offsets[j], seq_offsets[j+1]) (j < n_seq, seq_offsets[0]=0,
  *   seq_offsets[n_seq]=M) form group j, kept in input order, no merge, no drop; every string of

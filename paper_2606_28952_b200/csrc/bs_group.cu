@@ -62,7 +62,9 @@ __global__ void k_merge_runs(const i64* __restrict__ start, const u32* __restric
     xu[r] = xs[b];
     zu[r] = zs[b];
     cu[r] = make_double2(re, im);
-    keep[r] = (hypot(re, im) < eps) ? 0 : 1;  // drop |c| < eps_drop
+    // drop |c| < eps_drop; a merged coefficient that is exactly zero is dropped even with eps_drop = 0
+    const double a = hypot(re, im);
+    keep[r] = (a < eps || !(a > 0.0)) ? 0 : 1;
 }
 
 __global__ void k_compact(const int* __restrict__ keep, const int* __restrict__ pos, const u64* __restrict__ xu,

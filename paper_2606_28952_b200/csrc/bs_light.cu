@@ -21,19 +21,20 @@
 
 namespace {
 
-constexpr int kLT = 1024;   // threads per block
-constexpr int kLC = 4;      // columns per thread: column = tid + k * kLT
-constexpr int kLW = kLT * kLC;
+constexpr int kLC = 4;         // columns per thread: column = tid + k * T, T = threads per block
+constexpr int kLTmax = 1024;   // T = D_beta / 4 rounded up to a warp: no idle warps (3432 columns -> 864 threads)
 
-__device__ __forceinline__ u32 light_slot(u32 col) { return (col % kLT) * kLC + col / kLT; }
+__device__ __forceinline__ u32 light_slot(u32 col, u32 T) { return (col % T) * kLC + col / T; }
 
-// list build: entry j of a column = j-th valid listed table (source column | sign << 15), padded with D_beta
-// (the zero amplitude kept behind each staged row)
+// list build: entry j of a column = j-th valid listed table as (source column * 16) | sign -- the byte offset of the
+// source amplitude in the staged row with the sign in the free low bits -- padded with D_beta * 16 (the zero amplitude
+// kept behind each staged row).  D_beta <= 4094 keeps it in 16 bits.
 __global__ void k_light_list(SpinTab B, const uint2* __restrict__ tkeys, int n_listed, int l_max, int allow_by_table,
-                             unsigned short* __restrict__ L, int* __restrict__ cnt) {
+                             int T, unsigned short* __restrict__ L, int* __restrict__ cnt) {
     const u32 col = blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= (u32)kLW) return;
-    const u32 slot = light_slot(col);
+    const u32 kLW = (u32)T * kLC;
+    if (col >= kLW) return;
+    const u32 slot = light_slot(col, (u32)T);
     // When some column uses every listed table (l_max == n_listed: the Hubbard chain) compaction saves nothing, and
     // slot t = table t keeps the lanes of a warp on the same hop: neighbouring targets then read neighbouring sources
     // (fewer shared-memory bank conflicts than the compacted order, which mixes hops across lanes).
@@ -47,12 +48,12 @@ __global__ void k_light_list(SpinTab B, const uint2* __restrict__ tkeys, int n_l
             if (!valid && !(l_max && by_table)) continue;
             if (l_max)
                 L[(i64)j * kLW + slot] =
-                    valid ? (unsigned short)(spin_rank(B, tb ^ k.x) | ((u32)(__popc(tb & k.y) & 1) << 15)) : (unsigned short)B.D;
+                    valid ? (unsigned short)((spin_rank(B, tb ^ k.x) << 4) | (u32)(__popc(tb & k.y) & 1)) : (unsigned short)(B.D << 4);
             ++j;
         }
     }
     if (!l_max) cnt[col] = j;
-    else for (; j < l_max; ++j) L[(i64)j * kLW + slot] = (unsigned short)B.D;
+    else for (; j < l_max; ++j) L[(i64)j * kLW + slot] = (unsigned short)(B.D << 4);
 }
 
 // V table: for row r the keys of the x_a = 0 header, then one value per simple entry (in entry order)
@@ -76,8 +77,9 @@ __global__ void k_light_v(RowPlanDev P, u32 key0, u32 key1, const i64* __restric
     }
 }
 
-template <int MODE>  // 0: final epilogue, 2: expectation partials
-__global__ void __launch_bounds__(kLT, 1)
+template <int MODE, int MAXT, bool SIGN>  // MODE 0: final epilogue, 2: expectation partials; MAXT: launch bound (register
+                                         // budget); SIGN: some list entry carries a sign (else: plain sums, e.g. NN hops)
+__global__ void __launch_bounds__(MAXT, 1)
 k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__ out, i64 row_lo, i64 row_hi, Epilogue ep,
         double2* __restrict__ partials) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -87,8 +89,8 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
     u64* bar = reinterpret_cast<u64*>(smem_raw);
     double2* rowbuf = reinterpret_cast<double2*>(smem_raw + 16);           // [2][Db + 1]
     unsigned short* slist = reinterpret_cast<unsigned short*>(smem_raw + 16 + 2 * (size_t)(Db + 1) * 16);
-    double* slut = reinterpret_cast<double*>(smem_raw + 16 + 2 * (size_t)(Db + 1) * 16 + (size_t)L.l_max * kLW * 2);  // [2][8][16]
-    const u32 tid = threadIdx.x;
+    double* slut = reinterpret_cast<double*>(smem_raw + 16 + 2 * (size_t)(Db + 1) * 16 + (size_t)L.l_max * (blockDim.x * kLC) * 2);  // [2][8][16]
+    const u32 tid = threadIdx.x, kLT = blockDim.x, kLW = kLT * kLC;
     // rows are dealt round-robin (block b takes rows lo + b, lo + b + grid, ...): at any time the running rows
     // are ~grid consecutive ones, so the alpha-hop source rows (near neighbours in rank) stay L2-resident
     const i64 r0 = row_lo + (i64)blockIdx.x, r1 = row_hi, rs = gridDim.x;
@@ -107,7 +109,7 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
         {   // column list -> shared memory (8 bytes per thread and slot, conflict free)
             const uint2* __restrict__ src = reinterpret_cast<const uint2*>(L.llist);
             uint2* dst = reinterpret_cast<uint2*>(slist);
-            for (int i = tid; i < L.l_max * kLT; i += kLT) dst[i] = __ldg(src + i);
+            for (u32 i = tid; i < (u32)L.l_max * kLT; i += kLT) dst[i] = __ldg(src + i);
         }
         auto stage = [&](i64 r, u32 b) {  // thread 0 only
             const u32 bytes = Db * 16u;
@@ -154,7 +156,7 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
         const uint4* __restrict__ items4 = reinterpret_cast<const uint4*>(P.items);
         const u32 nk0 = reinterpret_cast<const u32*>(P.xa_hdr)[3] - L.key0;  // keys of the x_a = 0 header (header 0)
         const u32 wid = tid >> 5;
-        const bool alpha_first = L.order == 1 ? (wid & 1u) : L.order == 2 ? (wid >= kLT / 64) : L.order == 3 ? ((wid >> 2) & 1u) : false;
+        const bool alpha_first = L.order == 1 ? (wid & 1u) : L.order == 2 ? (wid >= kLT / 64u) : L.order == 3 ? ((wid >> 2) & 1u) : false;
         u32 it_n = 0;
         for (i64 r = r0; r < r1; r += rs, ++it_n) {
             const u32 b = it_n & 1u;
@@ -218,14 +220,15 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
             if (L.l_max > 0) {
                 const double vu = __ldg(Vr + (L.key_split - L.key0));
                 const uint2* __restrict__ sl = reinterpret_cast<const uint2*>(slist) + tid;
+                const unsigned char* __restrict__ sbytes = reinterpret_cast<const unsigned char*>(srow);
 #pragma unroll 4
                 for (int s = 0; s < L.l_max; ++s) {
-                    const uint2 e = sl[s * kLT];
+                    const uint2 e = sl[(u32)s * kLT];
                     const u32 en[kLC] = {e.x & 0xFFFFu, e.x >> 16, e.y & 0xFFFFu, e.y >> 16};
 #pragma unroll
                     for (int k = 0; k < kLC; ++k) {
-                        const double2 a = srow[en[k] & 0x7FFFu];
-                        const double f = flip(vu, en[k] >> 15);
+                        const double2 a = *reinterpret_cast<const double2*>(sbytes + (SIGN ? (en[k] & 0xFFF0u) : en[k]));
+                        const double f = SIGN ? flip(vu, en[k] & 1u) : vu;
                         acc[k].x += f * a.x;
                         acc[k].y += f * a.y;
                     }
@@ -281,8 +284,9 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
             for (int k = 0; k < kLC; ++k) {
                 if (!ok[k]) continue;
                 const i64 idx = r * (i64)Db + col[k];
-                if (L.stream) finish_target<MODE == 2, true>(acc[k], srow[col[k]], idx, out, ep, dot);
-                else finish_target<MODE == 2, false>(acc[k], srow[col[k]], idx, out, ep, dot);
+                const double2 pin = srow[col[k]];
+                if (L.stream) finish_target<MODE == 2, true>(acc[k], pin, idx, out, ep, dot);
+                else finish_target<MODE == 2, false>(acc[k], pin, idx, out, ep, dot);
             }
             __syncthreads();  // everyone is done with buffer b before row r + 2 is staged into it
         }
@@ -295,13 +299,29 @@ k_light(const LightDev L, const double2* __restrict__ psi, double2* __restrict__
 
 }  // namespace
 
+// Test hooks (include/bs.h "Environment"), read ONCE when the plan is built and stored in it.
+static int env_int(const char* name, int dflt) {
+    const char* v = getenv(name);
+    return v ? atoi(v) : dflt;
+}
+
+template <int MODE, bool SIGN>
+static cudaError_t light_set_smem(int maxt, size_t smem) {
+    switch (maxt) {
+        case 512: return cudaFuncSetAttribute(k_light<MODE, 512, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        case 768: return cudaFuncSetAttribute(k_light<MODE, 768, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        case 896: return cudaFuncSetAttribute(k_light<MODE, 896, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        default: return cudaFuncSetAttribute(k_light<MODE, 1024, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    }
+}
+
 // Decides whether the plan has the light shape and builds the shared-memory list image and the V table.
 int bs_light_build(bs_rowplan* R, cudaStream_t st) {
     R->light = false;
     if (getenv("BS_NO_LIGHT")) return BS_OK;
     const RowPlanDev& P = R->dev;
     const i64 Da = P.A.D, Db = P.B.D;
-    if (!R->real_w || Db > kLW || Db < 64 || R->h_hdrs.empty() || R->h_xa[0] != 0) return BS_OK;
+    if (!R->real_w || Db > 4094 || Db < 64 || R->h_hdrs.empty() || R->h_xa[0] != 0) return BS_OK;
     const XaHdr& h0 = R->h_hdrs[0];
     const bool listed = h0.item_split < h0.item1;
     if (listed && !(h0.stage & 2u)) return BS_OK;                 // the list must be uniform
@@ -310,6 +330,10 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
         if (R->h_items[i].tkey != kTkeyIdent) return BS_OK;       // dense part: diagonal-type groups only
     for (size_t x = 1; x < R->h_hdrs.size(); ++x)
         if (!R->h_hdrs[x].simple) return BS_OK;                   // every other alpha mask: a plain row axpy
+    // threads per block: a quarter of the columns, rounded up to a warp (BS_LIGHT_THREADS overrides: tests)
+    int T = (int)(((Db + kLC - 1) / kLC + 31) / 32 * 32);
+    if (int t = env_int("BS_LIGHT_THREADS", 0)) T = std::max(T, std::min(kLTmax, (t + 31) / 32 * 32));
+    const int kLW = T * kLC;
     // listed tables must be the first n_listed ones and all used by header 0 (true by construction)
     const int n_listed = listed ? R->n_listed : 0;
     DevBuf<uint2> d_tk;
@@ -319,7 +343,7 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
         std::vector<uint2> tk(R->h_tkeys.begin(), R->h_tkeys.begin() + n_listed);
         BS_CUDA(d_tk.upload(tk, st));
         BS_CUDA(d_cnt.alloc(kLW));
-        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, 0, 0, nullptr, d_cnt.p);
+        k_light_list<<<(kLW + 255) / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, 0, 0, T, nullptr, d_cnt.p);
         std::vector<int> hc(kLW);
         BS_CUDA(cudaMemcpyAsync(hc.data(), d_cnt.p, kLW * 4, cudaMemcpyDeviceToHost, st));
         BS_CUDA(cudaStreamSynchronize(st));
@@ -328,11 +352,16 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
     const size_t smem = 16 + 2 * (size_t)(Db + 1) * 16 + (size_t)l_max * kLW * 2 + 2 * 128 * 8;
     if (smem > 227 * 1024 - 1024) return BS_OK;
     BS_CUDA(R->d_llist.alloc((size_t)std::max(1, l_max) * kLW));
+    // slot t = table t for every column when some column uses every table (no compaction: see k_light_list);
+    // BS_LIGHT_COMPACT (test hook) compacts anyway
     if (l_max > 0) {
-        k_light_list<<<kLW / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, l_max, getenv("BS_LIGHT_COMPACT") ? 0 : 1, R->d_llist.p,
-                                                d_cnt.p);
+        k_light_list<<<(kLW + 255) / 256, 256, 0, st>>>(P.B, d_tk.p, n_listed, l_max, getenv("BS_LIGHT_COMPACT") ? 0 : 1, T,
+                                                        R->d_llist.p, d_cnt.p);
         BS_COUNT_LAUNCH(2);
     }
+    bool any_sign = false;   // a sign needs a listed table with z_b0 != 0 (NN hops of a chain have none)
+    for (int t = 0; t < n_listed; ++t) any_sign |= R->h_tkeys[t].y != 0;
+    R->light_sign = any_sign || env_int("BS_LIGHT_SIGN", 0);
     // V table
     std::vector<i64> roff(Da + 1), voff(Da + 1, 0);
     BS_CUDA(cudaMemcpyAsync(roff.data(), R->d_row_off.p, (Da + 1) * 8, cudaMemcpyDeviceToHost, st));
@@ -350,6 +379,26 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
     BS_COUNT_LAUNCH(1);
     BS_CUDA(cudaGetLastError());
     BS_CUDA(cudaStreamSynchronize(st));
+    // launch configuration, fixed here: the launch path below does nothing but launch
+    int dev = 0;
+    BS_CUDA(cudaGetDevice(&dev));
+    BS_CUDA(cudaDeviceGetAttribute(&R->light_sms, cudaDevAttrMultiProcessorCount, dev));
+    R->light_threads = T;
+    R->light_maxt = T <= 512 ? 512 : T <= 768 ? 768 : T <= 896 ? 896 : 1024;
+    R->light_stream = env_int("BS_LIGHT_STREAM", 1);
+    R->light_order = env_int("BS_LIGHT_ORDER", 3);  // 0: every warp runs the shared-memory phase first
+    R->light_lut_nq = 0;
+    if (h0.item_split - h0.item0 == 1) {
+        const u32 nk = R->h_items[h0.item0].nkeys;
+        if (nk >= 2 && nk <= 33) R->light_lut_nq = (int)((nk - 1 + 3) / 4);
+    }
+    if (R->light_sign) {
+        BS_CUDA((light_set_smem<0, true>(R->light_maxt, smem)));
+        BS_CUDA((light_set_smem<2, true>(R->light_maxt, smem)));
+    } else {
+        BS_CUDA((light_set_smem<0, false>(R->light_maxt, smem)));
+        BS_CUDA((light_set_smem<2, false>(R->light_maxt, smem)));
+    }
     R->light_lmax = l_max;
     R->light_smem = smem;
     R->light = true;
@@ -359,9 +408,6 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
 // rows [lo, hi) through the light kernel; expect: one dot partial per block
 int bs_light_apply(bs_rowplan* R, const double2* psi, double2* out, i64 lo, i64 hi, const Epilogue& ep, bool expect,
                    cudaStream_t st, double2* partials, i64* n_partials) {
-    int dev = 0, n_sm = 0;
-    BS_CUDA(cudaGetDevice(&dev));
-    BS_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     const XaHdr& h0 = R->h_hdrs[0];
     LightDev L;
     L.P = R->dev;
@@ -373,22 +419,28 @@ int bs_light_apply(bs_rowplan* R, const double2* psi, double2* out, i64 lo, i64 
     L.item_split = h0.item_split;
     L.key0 = h0.key0;
     L.key_split = h0.key_split;
-    L.stream = getenv("BS_LIGHT_STREAM") ? atoi(getenv("BS_LIGHT_STREAM")) : 1;
-    L.order = 3;
-    if (const char* o = getenv("BS_LIGHT_ORDER")) L.order = atoi(o);  // tuning: 0 = every warp runs the shared-memory phase first
-    L.lut_nq = 0;
-    if (h0.item_split - h0.item0 == 1) {
-        const u32 nk = R->h_items[h0.item0].nkeys;
-        if (nk >= 2 && nk <= 33) L.lut_nq = (int)((nk - 1 + 3) / 4);
+    L.stream = R->light_stream;
+    L.order = R->light_order;
+    L.lut_nq = R->light_lut_nq;
+    const unsigned grid = (unsigned)std::min<i64>(R->light_sms, hi - lo);
+    const unsigned T = (unsigned)R->light_threads;
+#define BS_LIGHT(M, MT)                                                                                             \
+    if (R->light_sign) k_light<M, MT, true><<<grid, T, R->light_smem, st>>>(L, psi, out, lo, hi, ep, expect ? partials : nullptr); \
+    else k_light<M, MT, false><<<grid, T, R->light_smem, st>>>(L, psi, out, lo, hi, ep, expect ? partials : nullptr)
+#define BS_LIGHT_MT(M)                                   \
+    switch (R->light_maxt) {                             \
+        case 512: BS_LIGHT(M, 512); break;               \
+        case 768: BS_LIGHT(M, 768); break;               \
+        case 896: BS_LIGHT(M, 896); break;               \
+        default: BS_LIGHT(M, 1024); break;               \
     }
-    const unsigned grid = (unsigned)std::min<i64>(n_sm, hi - lo);
     if (expect) {
-        BS_CUDA(cudaFuncSetAttribute(k_light<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->light_smem));
-        k_light<2><<<grid, kLT, R->light_smem, st>>>(L, psi, out, lo, hi, ep, partials);
+        BS_LIGHT_MT(2)
     } else {
-        BS_CUDA(cudaFuncSetAttribute(k_light<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->light_smem));
-        k_light<0><<<grid, kLT, R->light_smem, st>>>(L, psi, out, lo, hi, ep, nullptr);
+        BS_LIGHT_MT(0)
     }
+#undef BS_LIGHT_MT
+#undef BS_LIGHT
     BS_COUNT_LAUNCH(1);
     BS_CUDA(cudaGetLastError());
     if (n_partials) *n_partials = grid;

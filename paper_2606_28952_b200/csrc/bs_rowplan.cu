@@ -180,10 +180,12 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
             h.item_split = h.item1;
             h.key_split = h.key1;
         }
-    // stage bit 1: every listed group has a single string with z_a = 0 and the same weight
+    // stage bit 1: every listed group has a single string with z_a = 0 and the same weight -- AND the header owns
+    // every listed table: the column list is the union over all list-mode alpha masks, and the uniform pass ignores
+    // table ids, so a header with only a subset of the tables must take the sVx path (foreign tables: V = 0)
     for (auto& h : hdrs) {
         if (h.item_split >= h.item1) continue;
-        bool unif = true;
+        bool unif = (int)(h.item1 - h.item_split) == n_listed;
         const u32 s_first = key_s0[items[h.item_split].key0];
         for (u32 i = h.item_split; i < h.item1 && unif; ++i) {
             const u32 k = items[i].key0, sa = key_s0[k], sb = key_s0[k + 1];

@@ -93,7 +93,10 @@ struct bs_rowplan {
     bool light = false;
     int light_lmax = 0;
     size_t light_smem = 0;
-    DevBuf<unsigned short> d_llist;  // [light_lmax][4096], slot s of thread t: column t + 1024 * (s & 3) ...
+    int light_threads = 1024, light_maxt = 1024, light_sms = 0;        // launch geometry, fixed at plan build
+    int light_stream = 1, light_order = 3, light_lut_nq = 0, light_sign = 1;  // kernel switches (test hooks, read at plan build)
+    DevBuf<unsigned short> d_llist;  // [light_lmax][4 T], T = light_threads; entry 4 t + k of a slot: column t + k T;
+                                     // value = source column * 16 | sign
     DevBuf<double> d_vtab;           // V values, row after row
     DevBuf<i64> d_voff;              // [Da + 1]
 };

@@ -35,13 +35,35 @@ cases.append(('hub10', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 4))    
 cases.append(('hub10h', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 5))    # light path, list slots by table (l_max = 9 bonds)
 h, g = si.integrals(7, 77)
 cases.append(('mol7', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 7, 2, 5))
+# two list-mode alpha masks sharing one column list, the second uniform but owning only a SUBSET of the listed tables
+# (n = 10: NN and NNN beta hops with one weight under x_a = 0; V * (alpha hop 0-1) * (NN beta hop j) under x_a = {0,1})
+def _hop(P, Q, scale):
+    a = orc.ladder_product([P, Q], [1, 0], scale); b = orc.ladder_product([Q, P], [1, 0], scale)
+    return [a, b]
+parts = []
+for j in range(9): parts += _hop(10 + j, 11 + j, -1.0)
+for j in range(8): parts += _hop(10 + j, 12 + j, -1.0)
+for j in range(9):
+    for (P, Q) in ((0, 1), (1, 0)):
+        for (R, S) in ((10 + j, 11 + j), (11 + j, 10 + j)):
+            parts.append(orc.ladder_product([P, Q, R, S], [1, 0, 1, 0], 0.7))
+tl = (np.concatenate([p.x for p in parts]), np.concatenate([p.z for p in parts]), np.concatenate([p.c for p in parts]))
+# chain with nearest- and next-nearest-neighbour hops of equal weight on both spins + U n n: light-shaped, and the NNN
+# hops carry a JW sign (Z on the site in between), so the light kernel's signed list entries are exercised
+parts = []
+for sp in (0, 10):
+    for j in range(9): parts += _hop(sp + j, sp + j + 1, -1.0)
+    for j in range(8): parts += _hop(sp + j, sp + j + 2, -1.0)
+for j in range(10): parts.append(orc.ladder_product([j, j, 10 + j, 10 + j], [1, 0, 1, 0], 4.0))
+nnn = (np.concatenate([p.x for p in parts]), np.concatenate([p.z for p in parts]), np.concatenate([p.c for p in parts]))
 # generic complex operator (multi-key, POPC signs, complex weights)
 M = 400
 x = rng.integers(0, 1 << 12, M, dtype=np.uint64); x[:60] = 0; x[60:150] = 0b000011; x[150:260] = 0b000101000011
 x[260:300] = 0b011000000000
 z = rng.integers(0, 1 << 12, M, dtype=np.uint64)
 c = rng.standard_normal(M) + 1j * rng.standard_normal(M)
-for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2)]:
+for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2), ('twolist', None, tl, 10, 5, 5),
+                                        ('hubnnn', None, nnn, 10, 5, 4)]:
     op = bs.bs_group_xmask(*raw, 2 * n, 1e-12 if ref is not None else 0.0)
     if ref is None:
         xg, offs, zz, cc, _ = op.export()
@@ -49,7 +71,7 @@ for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2)]
     sec, osec = bs.bs_sector_build(n, na, nb), orc.Sector(n, na, nb)
     desc = bs.bs_plan_describe(op, sec)
     assert want_kernel in desc, (want_kernel, desc)
-    if name in ('hub10', 'hub10h') and want_kernel == 'rows_v2':
+    if name in ('hub10', 'hub10h', 'hubnnn') and want_kernel == 'rows_v2':
         assert ('+light' in desc) == (os.environ.get('BS_NO_LIGHT') is None), desc
     psi = si.random_state(osec.dim, 5)
     want = osec.apply_grouped(ref, psi) if osec.dim > 100000 else osec.apply(ref, psi)
@@ -77,8 +99,8 @@ print('PATH OK')
 @pytest.mark.parametrize("env,kernel", [
     ({}, "rows_v2"),
     ({"BS_NO_LIGHT": "1"}, "rows_v2"),
-    ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0"}, "rows_v2"),   # light kernel: compacted list, one phase order
-    ({"BS_LIGHT_ORDER": "1"}, "rows_v2"),
+    ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0", "BS_LIGHT_SIGN": "1"}, "rows_v2"),   # light kernel: compacted list, one phase order, signed entries
+    ({"BS_LIGHT_ORDER": "1", "BS_LIGHT_THREADS": "1024"}, "rows_v2"),
     ({"BS_KERNEL": "v1"}, "sector_v1"),
     ({"BS_KERNEL": "v2inrow"}, "kernel="),      # q24's beta-only groups do not fit in-row: falls back to v1 there
     ({"BS_ROW_WIN": "24"}, "n_win="),                                  # windowed rows, one column list per window
