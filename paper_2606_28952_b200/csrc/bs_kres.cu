@@ -1,0 +1,497 @@
+// a4, alpha-beta class resolved over (N_beta - 1)-electron strings: plan tables and the k_ab kernel.
+// See bs_kres.cuh for the formulation (Eq. 27-28; Eq. 23 for the JW chains).
+#include <algorithm>
+
+#include "bs_epilogue.cuh"
+#include "bs_kres.cuh"
+#include "bs_plan.cuh"
+
+namespace {
+
+// KresG codes: how one entry G[s][r] of a header's coupling matrix is made from the phase factors V_key(t_a)
+constexpr u32 kGSingle = 0u << 29;    // +-w (-1)^{popc(za & t_a)}: the group with x_b = {r, s} has one string (the JW case)
+constexpr u32 kGPair = 1u << 29;      // V(key) (bit 28: negated): the same with several strings
+constexpr u32 kGDiagKey = 2u << 29;   // sum_j V(dense key j) / N_beta - 2 V(dense key0 + low bits): x_b = 0 group, orbital carries a key
+constexpr u32 kGDiag = 3u << 29;      // sum_j V(dense key j) / N_beta
+constexpr u32 kGNone = 4u << 29;      // 0
+constexpr u32 kGType = 7u << 29;
+constexpr u32 kGNeg = 1u << 28;
+constexpr u32 kGKeyMask = (1u << 28) - 1;
+constexpr int kMaxDenseStr = 160;     // strings of an absorbed x_b = 0 group (3 n + 1 for a two-body Hamiltonian)
+constexpr int kMaxSegs = 48;          // staged column segments of a K chunk
+constexpr int kProducer = 32;         // threads of the producer warp (the last warp of the block)
+
+// register image of one header's tables in the producer warp, loaded one entry ahead of its use; the coupling-matrix
+// entries (lane, lane + 32, ...: at most NP of them) live in the registers the compute threads use as accumulators
+template <int NP>
+struct KresStage {
+    static constexpr int GQ = (NP * NP + 31) / 32, DQ = kMaxDenseStr / 32;
+    KresG d[DQ];   // strings of the absorbed x_b = 0 group (zero weight beyond the last)
+    u32 kr[2];     // string ranges (lo | hi << 8) of its keys lane and lane + 32
+};
+
+template <int NP, int KCMAX>
+__global__ void __launch_bounds__(KCMAX + kProducer, 1)
+k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S, i64 row_lo) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ double sVd[64], sStr[kMaxDenseStr];   // phase factors / signed string weights of the absorbed x_b = 0 group
+                                                     // (producer warp only)
+    __shared__ uint2 sSeg[kMaxSegs];
+    u64* bar = reinterpret_cast<u64*>(smem_raw);
+    double* sG = reinterpret_cast<double*>(smem_raw + 16);                                   // [2][NP * NP]
+    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 16 + 2 * NP * NP * 8);             // [2][buf_elems]
+    unsigned short* sgo =
+        reinterpret_cast<unsigned short*>(smem_raw + 16 + 2 * NP * NP * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
+    const int tid = threadIdx.x, KC = (int)blockDim.x - kProducer;
+    const bool producer = tid >= KC;
+    const int lane = tid & 31;
+    const i64 row = row_lo + blockIdx.x;
+    const int chunk = blockIdx.y;
+    const u32 ta = __ldg(Kd.a_str + row);
+    const int nseg = __ldg(Kd.seg_cnt + chunk);
+    u32 sig = 0;
+    if (!producer) {
+        sig = __ldg(Kd.sigma + (size_t)chunk * KC + tid);
+        for (int s = 0; s < NP; ++s) sgo[s * KC + tid] = __ldg(Kd.goff + ((size_t)chunk * NP + s) * KC + tid);
+    } else {
+        for (int g = lane; g < nseg; g += 32) sSeg[g] = __ldg(Kd.segs + (size_t)chunk * Kd.max_segs + g);
+    }
+    if (tid == KC) {
+        mbar_init(bar, 1);
+        mbar_init(bar + 1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        sbuf[0] = make_double2(0.0, 0.0);             // position 0 of either buffer: the zero amplitude (s in K)
+        sbuf[Kd.buf_elems] = make_double2(0.0, 0.0);
+    }
+    double2 acc[NP];
+#pragma unroll
+    for (int r = 0; r < NP; ++r) acc[r] = make_double2(0.0, 0.0);
+    const i64 e0 = __ldg(Kd.row_off + row);
+    const int n_ent = (int)(__ldg(Kd.row_off + row + 1) - e0);
+    const i64 Db = Kd.Db;
+    using Stage = KresStage<NP>;
+
+    // ---- producer warp -----------------------------------------------------------------------------------------
+    // all table loads of entry i (addresses depend on the header id only) into registers; consumed one entry later
+    auto load = [&](Stage& st, int i) {
+        const u32 kh = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i));
+        const KresG* __restrict__ gt = Kd.gtab + (size_t)kh * (NP * NP);
+#pragma unroll
+        for (int q = 0; q < Stage::GQ; ++q) {
+            const int p = lane + 32 * q;
+            if (p < NP * NP) acc[q] = *reinterpret_cast<const double2*>(gt + p);   // {w, (za, code)} as 16 raw bytes
+        }
+        const KresG* __restrict__ ds = Kd.dstr + (size_t)kh * kMaxDenseStr;
+#pragma unroll
+        for (int q = 0; q < Stage::DQ; ++q) st.d[q] = ds[lane + 32 * q];
+        const unsigned short* __restrict__ kr = Kd.dkr + (size_t)kh * 64;
+        st.kr[0] = __ldg(kr + lane);
+        st.kr[1] = __ldg(kr + lane + 32);
+    };
+    // TMA bulk copies of the chunk's column segments of entry i's source row into buffer i & 1 (lane 0)
+    auto stage_row = [&](int i) {
+        const u32 src_row = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i) + 1);
+        const double2* __restrict__ src = psi + (i64)src_row * Db;
+        unsigned char* dst = reinterpret_cast<unsigned char*>(sbuf + (size_t)(i & 1) * Kd.buf_elems + 1);
+        u32 total = 0;
+        for (int g = 0; g < nseg; ++g) total += sSeg[g].y * 16u;
+        mbar_expect_tx(bar + (i & 1), total);
+        for (int g = 0; g < nseg; ++g) {
+            const uint2 sg = sSeg[g];
+            const unsigned char* sp = reinterpret_cast<const unsigned char*>(src + sg.x);
+            const u32 bytes = sg.y * 16u;
+            for (u32 o = 0; o < bytes; o += 32768u) tma_bulk_g2s(dst + o, sp + o, min(32768u, bytes - o), bar + (i & 1));
+            dst += bytes;
+        }
+    };
+    // coupling matrix G[i & 1] of entry i from its register image
+    auto make_g = [&](const Stage& st, int i) {
+        double* G = sG + (i & 1) * (NP * NP);
+        // the absorbed x_b = 0 group: signed string weights, then one lane per key sums its strings in order;
+        // fixed-order butterfly for the total
+#pragma unroll
+        for (int q = 0; q < Stage::DQ; ++q) sStr[lane + 32 * q] = flip(st.d[q].w, (u32)__popc(st.d[q].za & ta) & 1u);
+        __syncwarp();
+        double dsum = 0.0;
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+            double v = 0.0;
+            for (u32 t = st.kr[jj] & 0xFFu; t < (st.kr[jj] >> 8); ++t) v += sStr[t];
+            sVd[lane + 32 * jj] = v;
+            dsum += v;
+        }
+        for (int o = 16; o > 0; o >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, o);
+        __syncwarp();
+        auto V = [&](u32 key) {   // groups with several strings per key (not the JW case): from the plan tables
+            double f = 0.0;
+            const u32 s1 = __ldg(Kd.key_s0 + key + 1);
+            for (u32 s = __ldg(Kd.key_s0 + key); s < s1; ++s)
+                f += flip(__ldg(&Kd.s_w[s].x), (u32)__popc(__ldg(Kd.s_za + s) & ta) & 1u);
+            return f;
+        };
+#pragma unroll
+        for (int q = 0; q < Stage::GQ; ++q) {
+            const int p = lane + 32 * q;
+            if (p >= NP * NP) break;
+            KresG g;
+            g.w = acc[q].x;
+            g.za = (u32)__double2loint(acc[q].y);
+            g.code = (u32)__double2hiint(acc[q].y);
+            const u32 type = g.code & kGType;
+            double v = 0.0;
+            if (type == kGSingle) v = flip(g.w, (u32)__popc(g.za & ta) & 1u);
+            else if (type == kGPair) {
+                v = V(g.code & kGKeyMask);
+                if (g.code & kGNeg) v = -v;
+            } else if (type == kGDiag) v = dsum * Kd.inv_nb;
+            else if (type == kGDiagKey) v = dsum * Kd.inv_nb - 2.0 * sVd[g.code & kGKeyMask];
+            G[p] = v;
+        }
+        __syncwarp();   // sStr / sVd are rewritten by the next entry
+    };
+    Stage st;
+    __syncthreads();
+    if (producer && n_ent > 0) {
+        load(st, 0);
+        if (lane == 0) stage_row(0);
+        make_g(st, 0);
+        if (n_ent > 1) load(st, 1);   // lands while the compute warps work on entry 0
+    }
+    __syncthreads();
+    for (int i = 0; i < n_ent; ++i) {
+        if (producer) {
+            // buffers (i + 1) & 1 were released by the barrier that ended entry i - 1
+            if (i + 1 < n_ent) {
+                if (lane == 0) stage_row(i + 1);
+                make_g(st, i + 1);
+                if (i + 2 < n_ent) load(st, i + 2);
+            }
+        } else {
+            mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
+            const double* __restrict__ G = sG + (i & 1) * (NP * NP);
+            const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
+#pragma unroll 2
+            for (int s = 0; s < Kd.n; ++s) {
+                double2 b = buf[sgo[s * KC + tid]];
+                const u32 sg = (sig >> s) & 1u;
+                b.x = flip(b.x, sg);
+                b.y = flip(b.y, sg);
+                const double2* __restrict__ g2 = reinterpret_cast<const double2*>(G + s * NP);
+#pragma unroll
+                for (int r2 = 0; r2 < NP / 2; ++r2) {
+                    const double2 g = g2[r2];   // warp-uniform address: one broadcast wavefront for two columns of G
+                    acc[2 * r2].x += g.x * b.x;
+                    acc[2 * r2].y += g.x * b.y;
+                    acc[2 * r2 + 1].x += g.y * b.x;
+                    acc[2 * r2 + 1].y += g.y * b.y;
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (producer) return;
+    double2* __restrict__ out = S + ((i64)blockIdx.x * Kd.n) * Kd.DKp + (i64)chunk * KC + tid;
+#pragma unroll
+    for (int r = 0; r < NP; ++r) {
+        if (r < Kd.n) {
+            const u32 sg = (sig >> r) & 1u;
+            out[(i64)r * Kd.DKp] = make_double2(flip(acc[r].x, sg), flip(acc[r].y, sg));
+        }
+    }
+}
+
+// compute threads + the producer warp fill whole groups of 4 warps (one per SM sub-partition): 512 threads at <= 128
+// registers for up to 16 orbitals, 256 threads at <= 255 registers above
+constexpr int kres_kcmax(int NP) { return NP <= 16 ? 480 : 224; }
+
+template <int NP>
+cudaError_t kab_launch(const bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st, bool set_attr) {
+    auto k = k_ab<NP, kres_kcmax(NP)>;
+    if (set_attr) return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K->smem);
+    dim3 grid((unsigned)(hi - lo), (unsigned)K->n_chunks);
+    k<<<grid, K->KC + kProducer, K->smem, st>>>(K->dev, psi, K->d_S.p, lo);
+    return cudaGetLastError();
+}
+
+cudaError_t kab_dispatch(const bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st, bool set_attr) {
+    switch (K->NP) {
+        case 8: return kab_launch<8>(K, psi, lo, hi, st, set_attr);
+        case 12: return kab_launch<12>(K, psi, lo, hi, st, set_attr);
+        case 16: return kab_launch<16>(K, psi, lo, hi, st, set_attr);
+        case 20: return kab_launch<20>(K, psi, lo, hi, st, set_attr);
+        case 24: return kab_launch<24>(K, psi, lo, hi, st, set_attr);
+        case 28: return kab_launch<28>(K, psi, lo, hi, st, set_attr);
+        default: return kab_launch<32>(K, psi, lo, hi, st, set_attr);
+    }
+}
+
+// all n-bit words of popcount k in increasing numeric order (k = 0: the empty string)
+std::vector<u32> subsets(int n, int k) {
+    std::vector<u32> out;
+    if (k == 0) {
+        out.push_back(0u);
+        return out;
+    }
+    u64 v = (u64(1) << k) - 1, lim = u64(1) << n;
+    while (v < lim) {
+        out.push_back((u32)v);
+        const u64 c = v & (~v + 1), r = v + c;   // next word with the same popcount
+        v = (((r ^ v) >> 2) / c) | r;
+    }
+    return out;
+}
+
+}  // namespace
+
+bs_kres::~bs_kres() { delete rp; }
+
+int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st, bs_kres** out) {
+    *out = nullptr;
+    if (getenv("BS_NO_KRES")) return BS_OK;   // test hook (include/bs.h "Environment")
+    const int n = S->n_orb, Nb = S->n_beta;
+    if (n < 5 || n > 32 || Nb < 1 || Nb >= n || S->Db < 64 || S->Db > 32767) return BS_OK;
+    // ---- which groups: under an alpha mask, the single-key beta single hops whose Z mask is the JW chain, and the
+    // x_b = 0 group when its beta Z masks are single bits (number operators) ------------------------------------
+    auto real_w = [](const HostGroup& g) {
+        for (auto& s : g.s)
+            if (s.im != 0.0) return false;
+        return true;
+    };
+    auto jw_hop = [&](const HostGroup& g) {
+        if (__builtin_popcount(g.xb) != 2 || g.s.front().zb != g.s.back().zb || !real_w(g)) return false;
+        const int lo = __builtin_ctz(g.xb), hi = 31 - __builtin_clz(g.xb);
+        const u32 between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
+        return (g.s.front().zb & ~g.xb) == between;
+    };
+    auto absorbable = [&](const HostGroup& g) {
+        if (g.xb != 0 || g.s.front().zb != 0 || !real_w(g)) return false;
+        for (auto& s : g.s)
+            if (s.zb != 0 && __builtin_popcount(s.zb) != 1) return false;
+        return true;
+    };
+    const int min_hops = getenv("BS_KRES_MIN") ? atoi(getenv("BS_KRES_MIN")) : 8;
+    std::map<u32, int> n_hops;
+    for (auto& g : groups)
+        if (g.xa != 0 && jw_hop(g)) ++n_hops[g.xa];
+    std::vector<HostGroup> mine, rest;
+    for (auto& g : groups) {
+        auto f = n_hops.find(g.xa);
+        const bool take = g.xa != 0 && f != n_hops.end() && f->second >= min_hops && (jw_hop(g) || absorbable(g));
+        (take ? mine : rest).push_back(g);
+    }
+    if (mine.empty()) return BS_OK;
+    bs_kres* K = new (std::nothrow) bs_kres;
+    BS_REQUIRE(K, BS_ERR_ALLOC, "kres plan allocation failed");
+    K->rp = new (std::nothrow) bs_rowplan;
+    int rc = K->rp ? bs_rowplan_build(K->rp, mine, S->ta, S->tb, st, false) : BS_ERR_ALLOC;
+    if (rc != BS_OK) {
+        delete K;
+        return rc;
+    }
+    const bs_rowplan* R = K->rp;
+    const int NP = (n + 3) & ~3;
+    K->n = n;
+    K->NP = NP;
+    K->Nb = Nb;
+    // ---- coupling-matrix tables -------------------------------------------------------------------------------
+    const size_t n_hdr = R->h_hdrs.size();
+    KresG none{};
+    none.code = kGNone;
+    std::vector<KresG> gtab(n_hdr * NP * NP, none);
+    std::vector<KresG> dstr(n_hdr * kMaxDenseStr, KresG{});   // strings of the absorbed group, zero weight beyond
+    std::vector<unsigned short> dkr(n_hdr * 64, 0);           // string range lo | hi << 8 of its keys (empty beyond)
+    for (size_t kh = 0; kh < n_hdr; ++kh) {
+        const XaHdr& h = R->h_hdrs[kh];
+        KresG* gm = gtab.data() + kh * NP * NP;
+        for (u32 i = h.item0; i < h.item1; ++i) {
+            const RowItem& it = R->h_items[i];
+            if (it.tkey == kTkeyIdent) {   // the absorbed x_b = 0 group: F = sum_j V_j (-1)^{n_q(j)} -> diagonal of G
+                const u32 d0 = R->h_key_s0[it.key0], d1 = R->h_key_s0[it.key0 + it.nkeys];
+                if (it.nkeys > 40 || d1 - d0 > (u32)kMaxDenseStr) {
+                    delete K;
+                    return BS_OK;
+                }
+                for (u32 t = d0; t < d1; ++t) {
+                    dstr[kh * kMaxDenseStr + (t - d0)].w = R->h_s_w[t].x;
+                    dstr[kh * kMaxDenseStr + (t - d0)].za = R->h_s_za[t];
+                }
+                for (u32 j = 0; j < it.nkeys; ++j)
+                    dkr[kh * 64 + j] = (unsigned short)((R->h_key_s0[it.key0 + j] - d0) | ((R->h_key_s0[it.key0 + j + 1] - d0) << 8));
+                for (int q = 0; q < n; ++q) gm[q * NP + q].code = kGDiag;
+                for (u32 j = 1; j < it.nkeys; ++j) {
+                    const int q = __builtin_ctz(R->h_key_dz[it.key0 + j]);
+                    gm[q * NP + q].code = kGDiagKey | j;
+                }
+            } else {
+                const uint2 tk = R->h_tkeys[it.tkey];   // {x_b, z_b0}
+                const int lo = __builtin_ctz(tk.x), hi = 31 - __builtin_clz(tk.x);
+                const u32 s0 = R->h_key_s0[it.key0], s1 = R->h_key_s0[it.key0 + 1];
+                // target K + {lo} <- source K + {hi}: the target holds lo, so z_b0's own bit on lo counts (and vice versa)
+                const int tgt[2] = {lo, hi}, src[2] = {hi, lo};
+                for (int d = 0; d < 2; ++d) {
+                    const bool neg = (tk.y >> tgt[d]) & 1u;
+                    KresG& e = gm[src[d] * NP + tgt[d]];
+                    if (s1 - s0 == 1) {
+                        e.w = neg ? -R->h_s_w[s0].x : R->h_s_w[s0].x;
+                        e.za = R->h_s_za[s0];
+                        e.code = kGSingle;
+                    } else e.code = kGPair | it.key0 | (neg ? kGNeg : 0u);
+                }
+            }
+        }
+    }
+    // ---- K strings, chunks, staged column segments ---------------------------------------------------------------
+    const std::vector<u32> Ks = subsets(n, Nb - 1);
+    const i64 DK = (i64)Ks.size();
+    K->DK = DK;
+    auto col_of = [&](u32 w) {
+        return (i64)(std::lower_bound(S->h_sb.begin(), S->h_sb.end(), (u64)w) - S->h_sb.begin());
+    };
+    const int kc_max = kres_kcmax(NP);   // register budget of k_ab<NP>
+    int KC = (int)std::min<i64>(kc_max, (DK + 31) / 32 * 32);
+    if (const char* e = getenv("BS_KRES_KC")) KC = std::max(32, std::min(kc_max, atoi(e) / 32 * 32));
+    const size_t smem_max = 227 * 1024 - 1024;
+    std::vector<uint2> segs;
+    std::vector<int> segcnt;
+    std::vector<unsigned short> goff;
+    int n_chunks = 0, max_segs = 0, buf_elems = 0;
+    double staged = 0;
+    for (;; KC /= 2) {
+        if (KC < 32) {
+            delete K;
+            return BS_OK;   // does not fit: the groups stay on the list path
+        }
+        n_chunks = (int)((DK + KC - 1) / KC);
+        std::vector<std::vector<uint2>> cs(n_chunks);
+        goff.assign((size_t)n_chunks * NP * KC, 0);
+        max_segs = 0;
+        buf_elems = 0;
+        staged = 0;
+        for (int c = 0; c < n_chunks; ++c) {
+            std::vector<u32> need;
+            for (i64 k = (i64)c * KC; k < std::min<i64>(DK, (i64)(c + 1) * KC); ++k)
+                for (int s = 0; s < n; ++s)
+                    if (!((Ks[k] >> s) & 1u)) need.push_back((u32)col_of(Ks[k] | (1u << s)));
+            std::sort(need.begin(), need.end());
+            need.erase(std::unique(need.begin(), need.end()), need.end());
+            std::vector<uint2>& sg = cs[c];
+            for (u32 gap = 32;; gap *= 2) {   // merge neighbouring columns into segments (few, long bulk copies)
+                sg.clear();
+                for (u32 v : need) {
+                    if (!sg.empty() && v <= sg.back().x + sg.back().y - 1 + gap) sg.back().y = v - sg.back().x + 1;
+                    else sg.push_back(make_uint2(v, 1u));
+                }
+                if (sg.size() <= (size_t)kMaxSegs) break;
+            }
+            std::vector<u32> base(sg.size());
+            u32 tot = 0;
+            for (size_t g = 0; g < sg.size(); ++g) {
+                base[g] = 1 + tot;   // position 0 is the zero amplitude
+                tot += sg[g].y;
+            }
+            buf_elems = std::max(buf_elems, (int)tot + 1);
+            staged += tot;
+            max_segs = std::max(max_segs, (int)sg.size());
+            for (i64 k = (i64)c * KC; k < std::min<i64>(DK, (i64)(c + 1) * KC); ++k)
+                for (int s = 0; s < n; ++s) {
+                    if ((Ks[k] >> s) & 1u) continue;
+                    const u32 col = (u32)col_of(Ks[k] | (1u << s));
+                    size_t g = std::upper_bound(sg.begin(), sg.end(), col, [](u32 v, const uint2& a) { return v < a.x; }) -
+                               sg.begin() - 1;
+                    goff[((size_t)c * NP + s) * KC + (k - (i64)c * KC)] = (unsigned short)(base[g] + (col - sg[g].x));
+                }
+        }
+        const size_t smem = 16 + 2 * (size_t)NP * NP * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
+        if (smem <= smem_max && buf_elems <= 65535) {
+            K->smem = smem;
+            segs.assign((size_t)n_chunks * max_segs, make_uint2(0u, 0u));
+            segcnt.resize(n_chunks);
+            for (int c = 0; c < n_chunks; ++c) {
+                segcnt[c] = (int)cs[c].size();
+                std::copy(cs[c].begin(), cs[c].end(), segs.begin() + (size_t)c * max_segs);
+            }
+            break;
+        }
+    }
+    K->KC = KC;
+    K->n_chunks = n_chunks;
+    K->max_segs = max_segs;
+    K->buf_elems = buf_elems;
+    K->DKp = (i64)n_chunks * KC;
+    K->staged_rows = staged / (double)S->Db;
+    std::vector<u32> sigma((size_t)K->DKp, 0u);
+    for (i64 k = 0; k < DK; ++k) {
+        u32 m = 0;
+        for (int p = 0; p < n; ++p) m |= ((u32)__builtin_popcount(Ks[k] & ((1u << p) - 1u)) & 1u) << p;
+        sigma[k] = m;
+    }
+    // ---- gather side: where the N_beta contributions of a target column sit in the scratch ---------------------
+    std::vector<u32> comb((size_t)S->Db * Nb);
+    for (i64 c = 0; c < S->Db; ++c) {
+        u32 tb = (u32)S->h_sb[c];
+        int j = 0;
+        for (u32 w = tb; w; w &= w - 1, ++j) {
+            const int r = __builtin_ctz(w);
+            const i64 kidx = std::lower_bound(Ks.begin(), Ks.end(), tb ^ (1u << r)) - Ks.begin();
+            comb[(size_t)c * Nb + j] = (u32)((i64)r * K->DKp + kidx);
+        }
+    }
+    if ((i64)n * K->DKp >= (i64(1) << 31)) {
+        delete K;
+        return BS_OK;
+    }
+    const i64 per_row = (i64)n * K->DKp * 16;
+    i64 budget = i64(4) << 30;
+    if (const char* e = getenv("BS_KRES_SLAB_MB")) budget = std::max<i64>(1, atoll(e)) << 20;   // test hook
+    K->slab_rows = std::max<i64>(1, std::min<i64>(S->Da, budget / per_row));
+    cudaError_t ce = K->d_S.alloc((size_t)(K->slab_rows * n * K->DKp));
+    if (ce == cudaSuccess) ce = K->d_gtab.upload(gtab, st);
+    if (ce == cudaSuccess) ce = K->d_dstr.upload(dstr, st);
+    if (ce == cudaSuccess) ce = K->d_dkr.upload(dkr, st);
+    if (ce == cudaSuccess) ce = K->d_goff.upload(goff, st);
+    if (ce == cudaSuccess) ce = K->d_sigma.upload(sigma, st);
+    if (ce == cudaSuccess) ce = K->d_segs.upload(segs, st);
+    if (ce == cudaSuccess) ce = K->d_segcnt.upload(segcnt, st);
+    if (ce == cudaSuccess) ce = K->d_comb.upload(comb, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    KresDev& d = K->dev;
+    d.row_off = R->d_row_off.p;
+    d.row_ent = R->d_row_ent.p;
+    d.a_str = S->ta.str;
+    d.gtab = K->d_gtab.p;
+    d.dstr = K->d_dstr.p;
+    d.dkr = K->d_dkr.p;
+    d.key_s0 = R->d_key_s0.p;
+    d.s_za = R->d_s_za.p;
+    d.s_w = R->d_s_w.p;
+    d.goff = K->d_goff.p;
+    d.sigma = K->d_sigma.p;
+    d.segs = K->d_segs.p;
+    d.seg_cnt = K->d_segcnt.p;
+    d.max_segs = max_segs;
+    d.KC = KC;
+    d.n_chunks = n_chunks;
+    d.n = n;
+    d.Nb = Nb;
+    d.buf_elems = buf_elems;
+    d.Db = S->Db;
+    d.DKp = K->DKp;
+    d.inv_nb = 1.0 / (double)Nb;
+    if (ce == cudaSuccess) ce = kab_dispatch(K, nullptr, 0, 0, st, true);
+    if (ce != cudaSuccess) {
+        bs_set_error("kres plan: %s", cudaGetErrorString(ce));
+        cudaGetLastError();
+        delete K;
+        return ce == cudaErrorMemoryAllocation ? BS_ERR_ALLOC : BS_ERR_CUDA;
+    }
+    groups.swap(rest);
+    *out = K;
+    return BS_OK;
+}
+
+// rows [lo, hi) (at most slab_rows) -> scratch S[row - lo][r][K]
+int bs_kres_apply(bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st) {
+    BS_CUDA(kab_dispatch(K, psi, lo, hi, st, false));
+    BS_COUNT_LAUNCH(1);
+    return BS_OK;
+}

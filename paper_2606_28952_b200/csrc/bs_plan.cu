@@ -5,6 +5,7 @@
 
 #include <algorithm>
 
+#include "bs_kres.cuh"
 #include "bs_plan.cuh"
 #include "bs_rowplan.cuh"
 
@@ -65,6 +66,14 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
         } else main_g.push_back(g);
     }
     std::stable_sort(t_g.begin(), t_g.end(), [](const HostGroup& a, const HostGroup& b) { return a.xa < b.xa; });
+    // alpha-beta groups with JW chains: K-resolved kernel (bs_kres.cuh); what it takes leaves main_g
+    bs_kres* kres = nullptr;
+    if (bs_kres_build(main_g, S, st, &kres) != BS_OK) {
+        cudaGetLastError();
+        kres = nullptr;
+        P->rows_fallback = 1;
+        return;
+    }
     bs_rowplan* m = new (std::nothrow) bs_rowplan;
     bs_rowplan* t = t_g.empty() ? nullptr : new (std::nothrow) bs_rowplan;
     bool ok = m && (t_g.empty() || t);
@@ -74,11 +83,14 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
         cudaGetLastError();
         bs_rowplan_free(m);
         bs_rowplan_free(t);
+        delete kres;
+        P->rows_fallback = 1;   // queryable: bs_plan_describe says "fallback=1"
         return;
     }
-    if (!t && bs_light_build(m, st) != BS_OK) cudaGetLastError();  // optional fast path; k_rows stays available
+    if (!t && !kres && bs_light_build(m, st) != BS_OK) cudaGetLastError();  // optional fast path; k_rows stays available
     P->rp_main = m;
     P->rp_t = t;
+    P->kres = kres;
 }
 
 int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
@@ -240,6 +252,7 @@ int bs_plan_get(bs_op* op, bs_sector* s, cudaStream_t st, bs_plan** out) {
 bs_plan::~bs_plan() {
     bs_rowplan_free(rp_main);
     bs_rowplan_free(rp_t);
+    delete kres;
 }
 void bs_rowplan_free(bs_rowplan* R) { delete R; }
 
@@ -269,6 +282,15 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
                          M->light ? "+light" : "", (int)M->real_w, M->n_xa, (long long)M->n_items, (long long)M->n_keys, (long long)M->n_strings,
                          (long long)M->n_tkeys, M->max_keys, (long long)M->n_row_ent, M->threads, M->cpt, M->chunk_cols,
                          M->win_cols, M->n_win, M->smem, M->n_listed, M->l_max);
+        if (P->kres && w > 0 && w < n) {
+            const bs_kres* K = P->kres;
+            w += snprintf(buf + w, (size_t)(n - w),
+                          " kres{xa=%d keys=%lld DK=%lld KC=%d chunks=%d NP=%d smem=%zu staged_rows=%.2f max_segs=%d slab_rows=%lld "
+                          "scratch_MB=%.0f}",
+                          K->rp->n_xa, (long long)K->rp->n_keys, (long long)K->DK, K->KC, K->n_chunks, K->NP, K->smem,
+                          K->staged_rows, K->max_segs, (long long)K->slab_rows,
+                          (double)K->slab_rows * K->n * K->DKp * 16.0 / 1048576.0);
+        }
         if (T && w > 0 && w < n)
             snprintf(buf + w, (size_t)(n - w),
                      " transposed{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d row_ent=%lld threads=%d "

@@ -20,8 +20,9 @@ struct HostGroup {
 };
 
 struct bs_rowplan;
+struct bs_kres;
 int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const SpinTab& A, const SpinTab& B,
-                     cudaStream_t st);
+                     cudaStream_t st, bool with_tables = true);
 void bs_rowplan_free(bs_rowplan* R);
 
 struct bs_plan {
@@ -54,6 +55,8 @@ struct bs_plan {
     // ---- v2 row plans (bs_rowplan.cuh); null -> the v1 kernel is used --------------------------------
     bs_rowplan* rp_main = nullptr;  // D, A, AB groups (and B groups when they are few)
     bs_rowplan* rp_t = nullptr;     // B groups as A groups of the transposed problem (when they are many)
+    bs_kres* kres = nullptr;        // alpha-beta groups resolved over (N_beta - 1)-electron strings (bs_kres.cuh)
+    int rows_fallback = 0;          // 1: a v2 row plan could not be built (allocation, limits) and the v1 kernel runs
     DevBuf<double2> d_psi_t, d_out_t, d_raw;  // transposed input / output, raw H psi (lazily allocated)
 
     // partial sums of bs_expect, one per thread block of the apply grid

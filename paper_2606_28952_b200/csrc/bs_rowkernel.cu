@@ -18,6 +18,7 @@
 #include <algorithm>
 
 #include "bs_epilogue.cuh"
+#include "bs_kres.cuh"
 #include "bs_plan.cuh"
 #include "bs_rowplan.cuh"
 
@@ -379,29 +380,43 @@ __global__ void __launch_bounds__(256) k_transpose(const double2* __restrict__ i
         if (c0 + j < C && r0 + tx < R) out_t[(c0 + j) * R + r0 + tx] = tile[tx][j];
 }
 
-// Final pass when part of the operator ran on the transposed problem: for rows [row_lo, row_hi)
-//   H psi [r][c] = raw[r][c] + out_t[c][r], then the fused epilogue (store / axpby / dot partial).
-template <bool EXPECT>
+// Final pass when the operator ran in parts: for rows [row_lo, row_hi)
+//   H psi [r][c] = raw[r][c]  (+ out_t[c][r]: the part applied to the transposed problem, TRANS)
+//                             (+ the N_beta K-resolved alpha-beta contributions of the target, from the scratch: KC.comb)
+// then the fused epilogue (store / axpby / dot partial).
+template <bool EXPECT, bool TRANS>
 __global__ void __launch_bounds__(256)
 k_transpose_add_finish(const double2* raw, const double2* __restrict__ out_t,
                        const double2* __restrict__ psi, double2* out, i64 Da, i64 Db, i64 row_lo,
-                       i64 row_hi, Epilogue ep, double2* __restrict__ partials) {
+                       i64 row_hi, Epilogue ep, KresComb KC, double2* __restrict__ partials) {
     __shared__ double2 tile[32][33];
     __shared__ double2 sh_red[32];
     const i64 r0 = row_lo + (i64)blockIdx.y * 32, c0 = (i64)blockIdx.x * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    for (int j = ty; j < 32; j += 8)  // tile[j][tx] = out_t[c0 + j][r0 + tx]
-        if (c0 + j < Db && r0 + tx < row_hi) tile[j][tx] = out_t[(c0 + j) * Da + r0 + tx];
-    __syncthreads();
+    if (TRANS) {
+        for (int j = ty; j < 32; j += 8)  // tile[j][tx] = out_t[c0 + j][r0 + tx]
+            if (c0 + j < Db && r0 + tx < row_hi) tile[j][tx] = out_t[(c0 + j) * Da + r0 + tx];
+        __syncthreads();
+    }
     double2 dot = make_double2(0.0, 0.0);
     for (int j = ty; j < 32; j += 8) {
         const i64 r = r0 + j, c = c0 + tx;
         if (r < row_hi && c < Db) {
             const i64 idx = r * Db + c;
             double2 a = raw[idx];
-            const double2 b = tile[tx][j];
-            a.x += b.x;
-            a.y += b.y;
+            if (TRANS) {
+                const double2 b = tile[tx][j];
+                a.x += b.x;
+                a.y += b.y;
+            }
+            if (KC.comb) {
+                const double2* __restrict__ Sr = KC.S + (r - KC.slab_lo) * (i64)KC.n * KC.DKp;
+                for (int e = 0; e < KC.Nb; ++e) {   // fixed order: deterministic
+                    const double2 v = __ldg(Sr + __ldg(KC.comb + c * KC.Nb + e));
+                    a.x += v.x;
+                    a.y += v.y;
+                }
+            }
             double2 pin = make_double2(0.0, 0.0);
             if (EXPECT || ep.use_axpby) pin = psi[idx];
             finish_target<EXPECT>(a, pin, idx, out, ep, dot);
@@ -458,7 +473,7 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
                   bool expect, cudaStream_t st, i64* n_partials_out, double2** partials_out) {
     bs_rowplan* M = P->rp_main;
     const i64 Da = s->Da, Db = s->Db;
-    if (!P->rp_t && M->light) {
+    if (!P->rp_t && !P->kres && M->light) {
         if (expect && P->n_partials < 1024) {
             BS_CUDA(P->d_partials.alloc(1024));
             P->n_partials = 1024;
@@ -470,7 +485,7 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
         if (partials_out) *partials_out = P->d_partials.p;
         return BS_OK;
     }
-    if (!P->rp_t) {
+    if (!P->rp_t && !P->kres) {
         const i64 nblk = (hi - lo) * ((Db + M->chunk_cols - 1) / M->chunk_cols);
         if (expect && P->n_partials < nblk) {
             BS_CUDA(P->d_partials.alloc(nblk));
@@ -482,34 +497,64 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
         if (partials_out) *partials_out = P->d_partials.p;
         return BS_OK;
     }
-    // part of the operator (beta-only groups) runs on the transposed problem
-    if (!P->d_psi_t.p) BS_CUDA(P->d_psi_t.alloc(s->D));
-    if (!P->d_out_t.p) BS_CUDA(P->d_out_t.alloc(s->D));
+    // the operator runs in parts: beta-only groups on the transposed problem (rp_t), alpha-beta groups K-resolved (kres)
+    bs_rowplan* T = P->rp_t;
+    bs_kres* K = P->kres;
+    if (T && !P->d_psi_t.p) BS_CUDA(P->d_psi_t.alloc(s->D));
+    if (T && !P->d_out_t.p) BS_CUDA(P->d_out_t.alloc(s->D));
     double2* raw = out;
     if (expect || !ep.store_out) {
         if (!P->d_raw.p) BS_CUDA(P->d_raw.alloc(s->D));
         raw = P->d_raw.p;
     }
-    dim3 tg((unsigned)((Db + 31) / 32), (unsigned)((Da + 31) / 32));
-    k_transpose<<<tg, 256, 0, st>>>(psi, P->d_psi_t.p, Da, Db);
-    BS_COUNT_LAUNCH(1);
-    BS_CUDA(cudaGetLastError());
     Epilogue none = ep;
+    if (T) {
+        dim3 tg((unsigned)((Db + 31) / 32), (unsigned)((Da + 31) / 32));
+        k_transpose<<<tg, 256, 0, st>>>(psi, P->d_psi_t.p, Da, Db);
+        BS_COUNT_LAUNCH(1);
+        BS_CUDA(cudaGetLastError());
+    }
     BS_CUDA(launch_k_rows<MODE_RAW>(M, st, psi, raw, lo, hi, 0, Db, none, nullptr));
-    BS_CUDA(launch_k_rows<MODE_RAW>(P->rp_t, st, P->d_psi_t.p, P->d_out_t.p, 0, Db, lo, hi, none, nullptr));
-    dim3 fg((unsigned)((Db + 31) / 32), (unsigned)((hi - lo + 31) / 32));
-    const i64 nblk = (i64)fg.x * fg.y;
+    if (T) BS_CUDA(launch_k_rows<MODE_RAW>(T, st, P->d_psi_t.p, P->d_out_t.p, 0, Db, lo, hi, none, nullptr));
+    const unsigned fgx = (unsigned)((Db + 31) / 32);
+    const i64 nblk = (i64)fgx * ((hi - lo + 31) / 32 + (K ? (hi - lo) / K->slab_rows + 1 : 0));
     if (expect && P->n_partials < nblk) {
         BS_CUDA(P->d_partials.alloc(nblk));
         P->n_partials = nblk;
     }
-    if (expect)
-        k_transpose_add_finish<true><<<fg, 256, 0, st>>>(raw, P->d_out_t.p, psi, out, Da, Db, lo, hi, ep, P->d_partials.p);
-    else
-        k_transpose_add_finish<false><<<fg, 256, 0, st>>>(raw, P->d_out_t.p, psi, out, Da, Db, lo, hi, ep, nullptr);
-    BS_COUNT_LAUNCH(1);
-    BS_CUDA(cudaGetLastError());
-    if (n_partials_out) *n_partials_out = nblk;
+    // finishing pass, slab by slab when the K-resolved part needs its scratch
+    const i64 slab = K ? K->slab_rows : hi - lo;
+    i64 pdone = 0;
+    for (i64 r0 = lo; r0 < hi; r0 += slab) {
+        const i64 r1 = std::min(hi, r0 + slab);
+        KresComb kc{};
+        if (K) {
+            int rc = bs_kres_apply(K, psi, r0, r1, st);
+            if (rc != BS_OK) return rc;
+            kc.comb = K->d_comb.p;
+            kc.S = K->d_S.p;
+            kc.Nb = K->Nb;
+            kc.n = K->n;
+            kc.DKp = K->DKp;
+            kc.slab_lo = r0;
+        }
+        dim3 fg(fgx, (unsigned)((r1 - r0 + 31) / 32));
+        double2* part = expect ? P->d_partials.p + pdone : nullptr;
+        const double2* ot = T ? P->d_out_t.p : nullptr;
+#define BS_FINISH(E, TR) k_transpose_add_finish<E, TR><<<fg, 256, 0, st>>>(raw, ot, psi, out, Da, Db, r0, r1, ep, kc, part)
+        if (expect) {
+            if (T) BS_FINISH(true, true);
+            else BS_FINISH(true, false);
+        } else {
+            if (T) BS_FINISH(false, true);
+            else BS_FINISH(false, false);
+        }
+#undef BS_FINISH
+        BS_COUNT_LAUNCH(1);
+        BS_CUDA(cudaGetLastError());
+        pdone += (i64)fg.x * fg.y;
+    }
+    if (n_partials_out) *n_partials_out = expect ? pdone : 0;
     if (partials_out) *partials_out = P->d_partials.p;
     return BS_OK;
 }

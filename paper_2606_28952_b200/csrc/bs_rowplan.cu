@@ -80,8 +80,10 @@ __global__ void k_row_fill2(SpinTab A, const u32* __restrict__ xa, const XaHdr* 
 }  // namespace
 
 // groups: already z-reduced, oriented (xa = row-spin mask, xb = column-spin mask), sorted by (xa, xb).
+// with_tables = false: headers / items / keys / strings and the per-row alpha-mask lists only (the K-resolved alpha-beta
+// kernel of bs_kres.cu brings its own column tables): no list mode, no column tables.
 int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, const SpinTab& A, const SpinTab& B,
-                     cudaStream_t st) {
+                     cudaStream_t st, bool with_tables) {
     const i64 Da = A.D, Db = B.D;
     // ---- list mode: which alpha masks serve their single-key x_b != 0 groups from the column list -------------
     auto listable = [](const HostGroup& g) { return g.xb != 0 && g.s.front().zb == g.s.back().zb; };
@@ -89,7 +91,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     for (auto& g : groups_in) n_listable[g.xa] += listable(g) ? 1 : 0;
     std::map<std::pair<u32, u32>, u32> listed_id;  // (xb, zb0) -> table id, listed tables first
     std::map<u32, bool> list_mode;
-    for (auto& kv : n_listable) list_mode[kv.first] = kv.second >= 8;
+    for (auto& kv : n_listable) list_mode[kv.first] = with_tables && kv.second >= 8;
     for (int pass = 0; pass < 2; ++pass) {
         listed_id.clear();
         for (auto& g : groups_in)
@@ -246,6 +248,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     R->n_chunks = n_chunks;
     R->chunk_cols = (int)chunk;
     R->tstride = (i64)R->n_chunks * R->threads * R->cpt;
+    if (!with_tables) R->tstride = 1;
     BS_REQUIRE((double)R->n_tkeys * (double)R->tstride * 2.0 <= 8e9, BS_ERR_ALLOC, "row plan: column tables too large");
     BS_REQUIRE(max_keys <= 2048, BS_ERR_ARG, "row plan: too many keys under one alpha mask");
     BS_CUDA(R->d_xa.upload(xa_list, st));
@@ -258,7 +261,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     DevBuf<uint2> d_tkeys;
     BS_CUDA(d_tkeys.upload(tkeys, st));
     BS_CUDA(R->d_ttab.alloc((size_t)std::max<i64>(1, R->n_tkeys) * R->tstride));
-    for (i64 k0 = 0; k0 < R->n_tkeys; k0 += 32768) {
+    for (i64 k0 = 0; with_tables && k0 < R->n_tkeys; k0 += 32768) {
         dim3 grid((unsigned)((R->tstride + 255) / 256), (unsigned)std::min<i64>(32768, R->n_tkeys - k0));
         k_fill_ttab<<<grid, 256, 0, st>>>(B, d_tkeys.p + k0, R->tstride, R->threads, R->cpt, R->chunk_cols,
                                           R->d_ttab.p + k0 * R->tstride);
@@ -270,6 +273,12 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     R->h_items = items;
     R->h_tkeys = tkeys;
     R->h_xa = xa_list;
+    R->h_key_dz = key_dz;
+    if (!with_tables) {   // the K-resolved plan folds single-string keys into its own tables
+        R->h_key_s0 = key_s0;
+        R->h_s_za = s_za;
+        R->h_s_w = s_w;
+    }
     R->l_max = 0;
     if (n_listed > 0) {
         DevBuf<int> lcnt;

@@ -86,6 +86,8 @@ struct bs_rowplan {
     std::vector<RowItem> h_items;
     std::vector<uint2> h_tkeys;  // {xb, zb0} of every column table, listed ones first
     std::vector<u32> h_xa;
+    std::vector<u32> h_key_dz, h_key_s0, h_s_za;
+    std::vector<double2> h_s_w;
     // ---- light path (bs_light.cu): few groups, HBM-bound operators such as lattice models ---------------------
     // One 1024-thread block per SM owns ALL columns of a strip of rows: the per-column hop list (u16 entries) lives
     // in shared memory for the whole launch, rows are double-buffered by TMA, and every phase factor V(t_a) is

@@ -35,6 +35,9 @@ cases.append(('hub10', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 4))    
 cases.append(('hub10h', ref10, jw.hubbard_raw_terms(10, 1.0, 4.0), 10, 5, 5))    # light path, list slots by table (l_max = 9 bonds)
 h, g = si.integrals(7, 77)
 cases.append(('mol7', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 7, 2, 5))
+h, g = si.integrals(9, 79)                                                          # n = 9 pads the K-resolved kernel's 12 columns
+cases.append(('mol9', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 9, 3, 5))
+cases.append(('mol9b', orc.molecular_h(h, g), jw.molecular_raw_terms(h, g), 9, 4, 2))
 # two list-mode alpha masks sharing one column list, the second uniform but owning only a SUBSET of the listed tables
 # (n = 10: NN and NNN beta hops with one weight under x_a = 0; V * (alpha hop 0-1) * (NN beta hop j) under x_a = {0,1})
 def _hop(P, Q, scale):
@@ -70,7 +73,9 @@ for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2),
         ref = orc.PauliOp(np.repeat(xg, np.diff(offs)), zz, cc)
     sec, osec = bs.bs_sector_build(n, na, nb), orc.Sector(n, na, nb)
     desc = bs.bs_plan_describe(op, sec)
-    assert want_kernel in desc, (want_kernel, desc)
+    assert want_kernel in desc or want_kernel == 'kres{', (want_kernel, desc)
+    if name in ('q24', 'mol9') and want_kernel in ('rows_v2', 'kres{'):
+        assert ('kres{' in desc) == (os.environ.get('BS_NO_KRES') is None), desc
     if name in ('hub10', 'hub10h', 'hubnnn') and want_kernel == 'rows_v2':
         assert ('+light' in desc) == (os.environ.get('BS_NO_LIGHT') is None), desc
     psi = si.random_state(osec.dim, 5)
@@ -98,7 +103,9 @@ print('PATH OK')
 
 @pytest.mark.parametrize("env,kernel", [
     ({}, "rows_v2"),
-    ({"BS_NO_LIGHT": "1"}, "rows_v2"),
+    ({"BS_NO_LIGHT": "1", "BS_NO_KRES": "1"}, "rows_v2"),             # column-list pass instead of the K-resolved kernel
+    ({"BS_KRES_KC": "64", "BS_KRES_SLAB_MB": "2"}, "kres{"),          # more K chunks, several scratch slabs
+    ({"BS_KRES_KC": "32", "BS_KRES_MIN": "1"}, "kres{"),
     ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0", "BS_LIGHT_SIGN": "1"}, "rows_v2"),   # light kernel: compacted list, one phase order, signed entries
     ({"BS_LIGHT_ORDER": "1", "BS_LIGHT_THREADS": "1024"}, "rows_v2"),
     ({"BS_KERNEL": "v1"}, "sector_v1"),
