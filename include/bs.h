@@ -28,9 +28,24 @@
  * stream); kernels are enqueued on it and the call returns without synchronising unless stated.
  * There is NO CPU fallback: without a CUDA device every compute entry point returns BS_ERR_CUDA.
  *
- * Threading: handles may be shared between host threads, but calls that use the same (operator, sector) pair
- * share library-owned scratch (cached plan, transposed copies, reduction partials) and must be issued on one
- * stream at a time.  Different pairs are independent.
+ * Threading: the library is not re-entrant per handle.  Calls that use the same operator handle OR the same sector
+ * handle share library-owned scratch (cached plan, transposed copies, K-resolution scratch, reduction partials and
+ * flags owned by the sector, rotation pair lists owned by the generator handle) and must be issued from one host
+ * thread on one stream at a time.  Pairs that share neither handle are independent.  One device per process.
+ *
+ * Library-owned device memory per (operator, sector) pair, allocated at the first bs_apply / bs_expect of the pair
+ * and freed with either handle (bs_plan_info reports the exact byte counts):
+ *   - plan tables (row lists: 16 B per valid (alpha row, alpha mask) pair; column tables; 1.2 GB at config 5);
+ *   - up to 3 state-vector-sized scratch buffers (transposed psi, transposed result, raw H psi) when beta-only
+ *     groups run on the transposed problem (every molecular Hamiltonian): 3 x 16 x dim bytes (20 GB at config 5);
+ *   - the scratch of the K-resolved alpha-beta kernel: n_orb x D_K x 16 bytes per alpha row of a slab, at most 4 GiB.
+ *
+ * Environment (TEST HOOKS, not API; every one is read ONCE, when a plan is built, never on a launch path):
+ *   BS_KERNEL=v1|v2inrow   force the v1 sector kernel / keep beta-only groups in-row
+ *   BS_NO_LIGHT, BS_LIGHT_THREADS, BS_LIGHT_ORDER, BS_LIGHT_STREAM, BS_LIGHT_COMPACT, BS_LIGHT_SIGN   k_light variants
+ *   BS_NO_KRES, BS_KRES_KC, BS_KRES_MIN, BS_KRES_SLAB_MB   K-resolved alpha-beta kernel off / chunk / threshold / slab
+ *   BS_ROW_WIN, BS_ROW_NO_SPLIT, BS_ROW_THREADS   k_rows source-row windows and block size
+ *   BS_ROT_PER_LAUNCH   one launch per rotation generator (no closed-cell batching); read per rotation call
  */
 #ifndef BS_H_
 #define BS_H_
@@ -136,6 +151,22 @@ int bs_apply_pauli_rotations(bs_op_t generators, bs_sector_t s, const double* th
 int bs_taylor_step(bs_op_t op, bs_sector_t s, void* psi_inout, void* work, double dt, int order,
                    double e_shift, void* cuda_stream);
 
+/* Machine-readable facts about the cached (op, sector) plan (built if needed); info [host] int64[8]:
+ *   [0] kernel path: 0 full space, 1 sector v1 (fallback), 2 row kernel v2, 3 v2 + light (few-group operators)
+ *   [1] 1 if a v2 row plan could NOT be built (allocation failure or a size limit) and the much slower v1 kernel runs
+ *   [2] 1 if beta-only groups run on the transposed problem   [3] 1 if alpha-beta groups run K-resolved
+ *   [4] bytes of state-vector-sized library scratch this pair can allocate (0, or 3 x 16 x dim)
+ *   [5] bytes of the K-resolution scratch (allocated at plan build)
+ *   [6] largest number of V slots (keys = distinct beta Z masks) under one alpha mask   [7] plan groups in total */
+int bs_plan_info(bs_op_t op, bs_sector_t s, int64_t info[8], void* cuda_stream);
+/* The groups of the plan after the spin split (Eq. 28) and the exact phase factorisation
+ * (Eq. 32-37): for group g, x[g] = its X mask (alpha bits | beta bits << n_orb) and nkeys[g] = the
+ * number of distinct beta Z masks of its strings, i.e. the number of terms of F_g(t_a, t_b) = sum_j V_gj(t_a)
+ * (-1)^{popc(zb_gj & t_b)} -- the exact counterpart of the paper's factorisation rank R_g (Table 1).
+ * x, nkeys [host] arrays of capacity cap (may be NULL to query); *n_groups receives the group count.  Sector mode with
+ * a v2 plan only (else BS_ERR_ARG). */
+int bs_plan_groups(bs_op_t op, bs_sector_t s, uint64_t* x, int32_t* nkeys, int64_t cap, int64_t* n_groups,
+                   void* cuda_stream);
 /* Human-readable description of the cached (op, sector) plan (kernel path, table sizes, launch
  * geometry) written to buf [host] (at most n bytes, NUL terminated); builds the plan if needed. */
 int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n, void* cuda_stream);

@@ -25,7 +25,7 @@ SYMBOLS = [
     "bs_group_xmask", "bs_op_info", "bs_op_export", "bs_op_destroy",
     "bs_sector_build", "bs_sector_info", "bs_sector_export", "bs_sector_rank", "bs_sector_destroy",
     "bs_apply", "bs_apply_rows", "bs_apply_axpby", "bs_expect", "bs_vdot",
-    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
+    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_plan_info", "bs_plan_groups", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
 ]
 
 
@@ -61,6 +61,8 @@ def _load():
     L.bs_jw_molecular.argtypes = [C.c_int, vp, vp, dbl, vp, C.POINTER(vp)]
     L.bs_jw_hubbard.argtypes = [C.c_int, dbl, dbl, dbl, vp, C.POINTER(vp)]
     L.bs_plan_describe.argtypes = [vp, vp, C.c_char_p, i64, vp]
+    L.bs_plan_info.argtypes = [vp, vp, C.POINTER(i64), vp]
+    L.bs_plan_groups.argtypes = [vp, vp, vp, vp, i64, C.POINTER(i64), vp]
     L.bs_launch_count.restype = i64
     L.bs_last_error.restype = C.c_char_p
     L.bs_version.restype = C.c_char_p
@@ -249,9 +251,30 @@ def bs_taylor_step(op: Op, sector: Sector, psi, work, dt: float, order: int = 12
 
 
 def bs_plan_describe(op: Op, sector: Sector, stream=None) -> str:
-    buf = C.create_string_buffer(1024)
-    _check(_lib.bs_plan_describe(op._h, sector._h, buf, 1024, _stream(stream)))
+    buf = C.create_string_buffer(2048)
+    _check(_lib.bs_plan_describe(op._h, sector._h, buf, 2048, _stream(stream)))
     return buf.value.decode()
+
+
+PLAN_INFO_FIELDS = ("kernel_path", "fallback", "transposed", "kres", "vector_scratch_bytes", "kres_scratch_bytes",
+                    "max_keys", "groups")
+
+
+def bs_plan_info(op: Op, sector: Sector, stream=None) -> dict:
+    """bs_plan_info as a dict (field names: PLAN_INFO_FIELDS)."""
+    info = (C.c_int64 * 8)()
+    _check(_lib.bs_plan_info(op._h, sector._h, info, _stream(stream)))
+    return dict(zip(PLAN_INFO_FIELDS, (int(v) for v in info)))
+
+
+def bs_plan_groups(op: Op, sector: Sector, stream=None):
+    """(x masks u64[G], key counts i32[G]) of the plan's groups (bs_plan_groups)."""
+    n = C.c_int64()
+    _check(_lib.bs_plan_groups(op._h, sector._h, None, None, 0, C.byref(n), _stream(stream)))
+    x = np.empty(n.value, np.uint64)
+    nk = np.empty(n.value, np.int32)
+    _check(_lib.bs_plan_groups(op._h, sector._h, _np_ptr(x), _np_ptr(nk), n.value, C.byref(n), _stream(stream)))
+    return x, nk
 
 
 def bs_jw_molecular(h, g, eps_drop: float = 1e-12, stream=None) -> Op:

@@ -37,11 +37,11 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
     __shared__ double sVd[64], sStr[kMaxDenseStr];   // phase factors / signed string weights of the absorbed x_b = 0 group
                                                      // (producer warp only)
     __shared__ uint2 sSeg[kMaxSegs];
-    u64* bar = reinterpret_cast<u64*>(smem_raw);
-    double* sG = reinterpret_cast<double*>(smem_raw + 16);                                   // [2][NP * NP]
-    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 16 + 2 * NP * NP * 8);             // [2][buf_elems]
+    u64* bar = reinterpret_cast<u64*>(smem_raw);   // full[2] (producer + TMA -> compute warps), empty[2] (compute warps -> producer)
+    double* sG = reinterpret_cast<double*>(smem_raw + 32);                                   // [2][NP * NP]
+    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 32 + 2 * NP * NP * 8);             // [2][buf_elems]
     unsigned short* sgo =
-        reinterpret_cast<unsigned short*>(smem_raw + 16 + 2 * NP * NP * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
+        reinterpret_cast<unsigned short*>(smem_raw + 32 + 2 * NP * NP * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
     const int tid = threadIdx.x, KC = (int)blockDim.x - kProducer;
     const bool producer = tid >= KC;
     const int lane = tid & 31;
@@ -49,16 +49,23 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
     const int chunk = blockIdx.y;
     const u32 ta = __ldg(Kd.a_str + row);
     const int nseg = __ldg(Kd.seg_cnt + chunk);
-    u32 sig = 0;
+    u32 sig = 0, in_k = 0;   // in_k: orbitals that every K of this warp holds (no source, no target there: skipped)
     if (!producer) {
         sig = __ldg(Kd.sigma + (size_t)chunk * KC + tid);
-        for (int s = 0; s < NP; ++s) sgo[s * KC + tid] = __ldg(Kd.goff + ((size_t)chunk * NP + s) * KC + tid);
+        for (int s = 0; s < NP; ++s) {
+            const unsigned short o = __ldg(Kd.goff + ((size_t)chunk * NP + s) * KC + tid);
+            sgo[s * KC + tid] = o;
+            in_k |= (o == 0 ? 1u : 0u) << s;
+        }
+        in_k = __reduce_and_sync(0xffffffffu, in_k);
     } else {
         for (int g = lane; g < nseg; g += 32) sSeg[g] = __ldg(Kd.segs + (size_t)chunk * Kd.max_segs + g);
     }
     if (tid == KC) {
-        mbar_init(bar, 1);
-        mbar_init(bar + 1, 1);
+        mbar_init(bar, 2);       // full: the producer arrives twice (byte count of the copies; G written)
+        mbar_init(bar + 1, 2);
+        mbar_init(bar + 2, (u32)KC / 32);
+        mbar_init(bar + 3, (u32)KC / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         sbuf[0] = make_double2(0.0, 0.0);             // position 0 of either buffer: the zero amplitude (s in K)
         sbuf[Kd.buf_elems] = make_double2(0.0, 0.0);
@@ -70,6 +77,7 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
     const int n_ent = (int)(__ldg(Kd.row_off + row + 1) - e0);
     const i64 Db = Kd.Db;
     using Stage = KresStage<NP>;
+    u32 seg_bytes = 0;   // producer: bytes of one entry's bulk copies
 
     // ---- producer warp -----------------------------------------------------------------------------------------
     // all table loads of entry i (addresses depend on the header id only) into registers; consumed one entry later
@@ -93,9 +101,7 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
         const u32 src_row = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i) + 1);
         const double2* __restrict__ src = psi + (i64)src_row * Db;
         unsigned char* dst = reinterpret_cast<unsigned char*>(sbuf + (size_t)(i & 1) * Kd.buf_elems + 1);
-        u32 total = 0;
-        for (int g = 0; g < nseg; ++g) total += sSeg[g].y * 16u;
-        mbar_expect_tx(bar + (i & 1), total);
+        mbar_expect_tx(bar + (i & 1), seg_bytes);
         for (int g = 0; g < nseg; ++g) {
             const uint2 sg = sSeg[g];
             const unsigned char* sp = reinterpret_cast<const unsigned char*>(src + sg.x);
@@ -112,11 +118,19 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
 #pragma unroll
         for (int q = 0; q < Stage::DQ; ++q) sStr[lane + 32 * q] = flip(st.d[q].w, (u32)__popc(st.d[q].za & ta) & 1u);
         __syncwarp();
+        // key 0 (beta Z mask 0) is the long one for a two-body Hamiltonian (n + 1 strings): the whole warp sums it;
+        // the other keys (one or two strings each) take one lane each
+        const u32 k0 = __shfl_sync(0xffffffffu, st.kr[0], 0);
+        double v0 = 0.0;
+        for (u32 t = (k0 & 0xFFu) + lane; t < (k0 >> 8); t += 32) v0 += sStr[t];
+        for (int o = 16; o > 0; o >>= 1) v0 += __shfl_xor_sync(0xffffffffu, v0, o);
         double dsum = 0.0;
 #pragma unroll
         for (int jj = 0; jj < 2; ++jj) {
             double v = 0.0;
-            for (u32 t = st.kr[jj] & 0xFFu; t < (st.kr[jj] >> 8); ++t) v += sStr[t];
+            if (jj == 0 && lane == 0) v = v0;
+            else
+                for (u32 t = st.kr[jj] & 0xFFu; t < (st.kr[jj] >> 8); ++t) v += sStr[t];
             sVd[lane + 32 * jj] = v;
             dsum += v;
         }
@@ -147,49 +161,60 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
             else if (type == kGDiagKey) v = dsum * Kd.inv_nb - 2.0 * sVd[g.code & kGKeyMask];
             G[p] = v;
         }
-        __syncwarp();   // sStr / sVd are rewritten by the next entry
+        __syncwarp();   // sStr / sVd are rewritten by the next entry; G is complete
+        // the producer's second arrival on full[i & 1] (release: G is visible to whoever observes the phase)
+        if (lane == 0) mbar_arrive(bar + (i & 1));
     };
     Stage st;
     __syncthreads();
-    if (producer && n_ent > 0) {
-        load(st, 0);
-        if (lane == 0) stage_row(0);
-        make_g(st, 0);
-        if (n_ent > 1) load(st, 1);   // lands while the compute warps work on entry 0
-    }
-    __syncthreads();
-    for (int i = 0; i < n_ent; ++i) {
-        if (producer) {
-            // buffers (i + 1) & 1 were released by the barrier that ended entry i - 1
-            if (i + 1 < n_ent) {
-                if (lane == 0) stage_row(i + 1);
-                make_g(st, i + 1);
-                if (i + 2 < n_ent) load(st, i + 2);
-            }
-        } else {
-            mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
-            const double* __restrict__ G = sG + (i & 1) * (NP * NP);
-            const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
-#pragma unroll 2
-            for (int s = 0; s < Kd.n; ++s) {
-                double2 b = buf[sgo[s * KC + tid]];
-                const u32 sg = (sig >> s) & 1u;
-                b.x = flip(b.x, sg);
-                b.y = flip(b.y, sg);
-                const double2* __restrict__ g2 = reinterpret_cast<const double2*>(G + s * NP);
-#pragma unroll
-                for (int r2 = 0; r2 < NP / 2; ++r2) {
-                    const double2 g = g2[r2];   // warp-uniform address: one broadcast wavefront for two columns of G
-                    acc[2 * r2].x += g.x * b.x;
-                    acc[2 * r2].y += g.x * b.y;
-                    acc[2 * r2 + 1].x += g.y * b.x;
-                    acc[2 * r2 + 1].y += g.y * b.y;
-                }
-            }
+    if (producer) {
+        // No block barrier in the entry loop: the producer refills buffer b as soon as every compute warp has released
+        // it (empty[b]); a compute warp starts entry i as soon as full[i & 1] completes, whatever the other warps do.
+        for (int g = 0; g < nseg; ++g) seg_bytes += sSeg[g].y * 16u;
+        if (n_ent > 0) load(st, 0);
+        for (int i = 0; i < n_ent; ++i) {
+            if (i >= 2) mbar_wait(bar + 2 + (i & 1), (u32)((i >> 1) - 1) & 1u);
+            if (lane == 0) stage_row(i);
+            make_g(st, i);
+            if (i + 1 < n_ent) load(st, i + 1);   // lands while this warp waits for the next free buffer
         }
-        __syncthreads();
+        return;
     }
-    if (producer) return;
+    // orbitals with a source K + {s} for some K of this warp, walked in ascending order (warp-uniform); the gather of
+    // the next orbital is issued before the DFMA block of the current one
+    const u32 act_all = ~in_k & (Kd.n >= 32 ? 0xFFFFFFFFu : ((1u << Kd.n) - 1u));
+    const unsigned short* __restrict__ my_go = sgo + tid;
+    for (int i = 0; i < n_ent; ++i) {
+        mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
+        const double* __restrict__ G = sG + (i & 1) * (NP * NP);
+        const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
+        u32 act = act_all;
+        int s = __ffs((int)act) - 1;
+        act &= act - 1;
+        double2 b = (s >= 0) ? buf[my_go[s * KC]] : make_double2(0.0, 0.0);
+        while (s >= 0) {
+            const int sn = __ffs((int)act) - 1;   // -1 when none is left
+            act &= act - 1;
+            double2 bn = make_double2(0.0, 0.0);
+            if (sn >= 0) bn = buf[my_go[sn * KC]];
+            const u32 sg = (sig >> s) & 1u;
+            b.x = flip(b.x, sg);
+            b.y = flip(b.y, sg);
+            const double2* __restrict__ g2 = reinterpret_cast<const double2*>(G + s * NP);
+#pragma unroll
+            for (int r2 = 0; r2 < NP / 2; ++r2) {
+                const double2 g = g2[r2];   // warp-uniform address: one broadcast wavefront for two columns of G
+                acc[2 * r2].x += g.x * b.x;
+                acc[2 * r2].y += g.x * b.y;
+                acc[2 * r2 + 1].x += g.y * b.x;
+                acc[2 * r2 + 1].y += g.y * b.y;
+            }
+            s = sn;
+            b = bn;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar + 2 + (i & 1));   // this warp is done with buffer i & 1
+    }
     double2* __restrict__ out = S + ((i64)blockIdx.x * Kd.n) * Kd.DKp + (i64)chunk * KC + tid;
 #pragma unroll
     for (int r = 0; r < NP; ++r) {
@@ -401,7 +426,7 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
                     goff[((size_t)c * NP + s) * KC + (k - (i64)c * KC)] = (unsigned short)(base[g] + (col - sg[g].x));
                 }
         }
-        const size_t smem = 16 + 2 * (size_t)NP * NP * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
+        const size_t smem = 32 + 2 * (size_t)NP * NP * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
         if (smem <= smem_max && buf_elems <= 65535) {
             K->smem = smem;
             segs.assign((size_t)n_chunks * max_segs, make_uint2(0u, 0u));

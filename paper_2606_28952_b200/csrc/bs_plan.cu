@@ -266,6 +266,53 @@ void bs_plan_purge(u64 op_id, u64 sector_id) {
     }
 }
 
+extern "C" int bs_plan_info(bs_op_t op, bs_sector_t s, int64_t info[8], void* cuda_stream) {
+    BS_REQUIRE(op && s && info, BS_ERR_ARG, "bs_plan_info: bad argument");
+    bs_plan* P = nullptr;
+    int rc = bs_plan_get(op, s, (cudaStream_t)cuda_stream, &P);
+    if (rc != BS_OK) return rc;
+    for (int i = 0; i < 8; ++i) info[i] = 0;
+    info[0] = P->full ? 0 : (!P->rp_main ? 1 : (P->rp_main->light && !P->rp_t && !P->kres ? 3 : 2));
+    info[1] = P->rows_fallback;
+    info[2] = P->rp_t ? 1 : 0;
+    info[3] = P->kres ? 1 : 0;
+    info[4] = (P->rp_t || P->kres) ? 3 * 16 * s->D : 0;
+    info[5] = P->kres ? (int64_t)P->kres->slab_rows * P->kres->n * P->kres->DKp * 16 : 0;
+    if (P->rp_main) {
+        info[6] = P->rp_main->max_keys;
+        info[7] = P->rp_main->n_items + (P->rp_t ? P->rp_t->n_items : 0) + (P->kres ? P->kres->rp->n_items : 0);
+    }
+    return BS_OK;
+}
+
+extern "C" int bs_plan_groups(bs_op_t op, bs_sector_t s, uint64_t* x, int32_t* nkeys, int64_t cap, int64_t* n_groups,
+                              void* cuda_stream) {
+    BS_REQUIRE(op && s && n_groups, BS_ERR_ARG, "bs_plan_groups: bad argument");
+    bs_plan* P = nullptr;
+    int rc = bs_plan_get(op, s, (cudaStream_t)cuda_stream, &P);
+    if (rc != BS_OK) return rc;
+    BS_REQUIRE(!P->full && P->rp_main, BS_ERR_ARG, "bs_plan_groups: needs a sector-mode v2 plan");
+    int64_t n = 0;
+    auto emit = [&](const bs_rowplan* R, bool transposed) {
+        if (!R) return;
+        for (size_t h = 0; h < R->h_hdrs.size(); ++h)
+            for (u32 i = R->h_hdrs[h].item0; i < R->h_hdrs[h].item1; ++i) {
+                const RowItem& it = R->h_items[i];
+                const u64 xr = R->h_xa[h], xc = it.tkey == kTkeyIdent ? 0u : R->h_tkeys[it.tkey].x;   // row / column spin
+                if (x && nkeys && n < cap) {
+                    x[n] = transposed ? (xc | (xr << s->n_orb)) : (xr | (xc << s->n_orb));
+                    nkeys[n] = (int32_t)it.nkeys;
+                }
+                ++n;
+            }
+    };
+    emit(P->rp_main, false);
+    emit(P->kres ? P->kres->rp : nullptr, false);
+    emit(P->rp_t, true);
+    *n_groups = n;
+    return BS_OK;
+}
+
 extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n, void* cuda_stream) {
     BS_REQUIRE(op && s && buf && n > 0, BS_ERR_ARG, "bs_plan_describe: bad argument");
     bs_plan* P = nullptr;
@@ -277,7 +324,7 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
         const bs_rowplan* M = P->rp_main;
         const bs_rowplan* T = P->rp_t;
         int w = snprintf(buf, (size_t)n,
-                         "kernel=rows_v2%s real_w=%d main{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d "
+                         "kernel=rows_v2%s fallback=0 real_w=%d main{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d "
                          "row_ent=%lld threads=%d cpt=%d chunk_cols=%d win_cols=%d n_win=%d smem=%zu listed=%d l_max=%d}",
                          M->light ? "+light" : "", (int)M->real_w, M->n_xa, (long long)M->n_items, (long long)M->n_keys, (long long)M->n_strings,
                          (long long)M->n_tkeys, M->max_keys, (long long)M->n_row_ent, M->threads, M->cpt, M->chunk_cols,
@@ -298,8 +345,9 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
                      T->n_xa, (long long)T->n_items, (long long)T->n_keys, (long long)T->n_strings, (long long)T->n_tkeys,
                      T->max_keys, (long long)T->n_row_ent, T->threads, T->cpt, T->chunk_cols, T->smem);
     } else {
-        snprintf(buf, (size_t)n, "kernel=sector_v1 real_w=%d xa=%d groups=%lld strings=%lld row_ent=%lld", (int)P->real_w,
-                 P->n_xa, (long long)P->n_groups, (long long)P->n_strings, (long long)P->n_row_ent);
+        snprintf(buf, (size_t)n, "kernel=sector_v1 fallback=%d real_w=%d xa=%d groups=%lld strings=%lld row_ent=%lld",
+                 P->rows_fallback, (int)P->real_w, P->n_xa, (long long)P->n_groups, (long long)P->n_strings,
+                 (long long)P->n_row_ent);
     }
     return BS_OK;
 }

@@ -428,22 +428,26 @@ k_transpose_add_finish(const double2* raw, const double2* __restrict__ out_t,
     }
 }
 
+// The opt-in shared-memory ceiling is raised ONCE per kernel instantiation (thread-safe static initialisation; the
+// library drives one device per process), not on every launch; occupancy follows the size actually launched.
+constexpr int kMaxDynSmem = 227 * 1024;
+
 template <int MODE, bool REALW, int CPT>
 cudaError_t launch_k_rows_t(const bs_rowplan* R, dim3 grid, cudaStream_t st, const double2* psi, double2* out,
                             i64 row_lo, i64 col_lo, i64 col_hi, int chunk0, const Epilogue& ep, double2* partials) {
     if (R->threads > 512) {
         auto k = k_rows<MODE, REALW, CPT, 1024>;
-        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        static const cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
         if (e != cudaSuccess) return e;
         k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
     } else if (R->threads > 256) {
         auto k = k_rows<MODE, REALW, CPT, 512>;
-        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        static const cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
         if (e != cudaSuccess) return e;
         k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
     } else {
         auto k = k_rows<MODE, REALW, CPT, 256>;
-        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R->smem);
+        static const cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
         if (e != cudaSuccess) return e;
         k<<<grid, R->threads, R->smem, st>>>(R->dev, psi, out, row_lo, col_lo, col_hi, chunk0, ep, partials);
     }

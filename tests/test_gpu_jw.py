@@ -26,7 +26,7 @@ def _check_tables(op, ref):
     assert np.abs(cc.imag).max() == 0.0            # every true coefficient of a real Hamiltonian is real (pin P3)
 
 
-@pytest.mark.parametrize("name", ["q12", "q24", "q32"])
+@pytest.mark.parametrize("name", ["q12", "q24", "q32", "q56"])   # q56: 3.9e7 raw strings, the route bench.py times
 def test_jw_molecular_tables(bs, name):
     cfg = si.CONFIGS[name]
     h, g = si.integrals(cfg.n_orb, cfg.seed_ints)

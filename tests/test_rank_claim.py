@@ -1,0 +1,90 @@
+"""The rank claim behind the paper's phase factorisation (Eq. 32-37; Table 1)
+checked on the synthetic integrals, and the library's exact factorisation set against it.
+
+CPU part: for every X-mask group g of the oracle's Hamiltonian, M^(g) (rows = distinct alpha Z masks, columns =
+distinct beta Z masks, entries = summed coefficients; Eq. 32) has numerical rank R_g <= 2 for x != 0 and
+R_0 = n_orb + 2 for the diagonal group (tolerance 1e-12 on the singular values, as in Table 1).
+
+GPU part: the plan keeps, per spin-split group, one term per DISTINCT beta Z mask ("key": bs_plan_groups).  That is an
+exact factorisation, not a minimal one: it equals the paper's rank (1) on the alpha-beta groups, which hold 71-72 % of
+the non-zeros, and exceeds it on the 2 C(n,2) single-excitation groups (n + 1 keys vs rank 2) and on the diagonal group
+(1 + n + C(n,2) keys vs rank n + 2), whose extra keys are single-bit sign flips evaluated once per row.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import synth_inputs as si
+from common import oracle_operator
+
+
+def _ranks(op, n):
+    ma = np.uint64((1 << n) - 1)
+    xs, first = np.unique(op.x, return_index=True)
+    bounds = list(first) + [len(op)]
+    out = {}
+    for g, x in enumerate(xs):
+        k0, k1 = bounds[g], bounds[g + 1]
+        za, zb = op.z[k0:k1] & ma, op.z[k0:k1] >> np.uint64(n)
+        ua, ia = np.unique(za, return_inverse=True)
+        ub, ib = np.unique(zb, return_inverse=True)
+        m = np.zeros((len(ua), len(ub)))
+        np.add.at(m, (ia, ib), op.c[k0:k1].real)                 # Eq. 32: coefficients summed per (Z_alpha, Z_beta)
+        sv = np.linalg.svd(m, compute_uv=False)
+        out[int(x)] = int((sv > 1e-12).sum())
+    return out
+
+
+@pytest.mark.parametrize("name", ["q12", "q24"])
+def test_rank_of_phase_matrices_on_synthetic_integrals(name):
+    cfg = si.CONFIGS[name]
+    n = cfg.n_orb
+    r = _ranks(oracle_operator(name), n)
+    assert r[0] == n + 2                                         # identity + one-body diagonal + n (cross-spin Coulomb)
+    off = np.array([v for x, v in r.items() if x != 0])
+    assert off.min() >= 1 and off.max() <= 2
+    # rank 2 exactly on the single-excitation groups (x on one spin, two bits): 2 C(n,2) of them
+    ma = (1 << n) - 1
+    two = {x for x, v in r.items() if v == 2}
+    singles = {x for x in r if x and bin(x).count("1") == 2 and ((x & ma) == 0 or (x >> n) == 0)}
+    assert two == singles and len(singles) == 2 * math.comb(n, 2)
+    mean = off.mean()
+    assert 1.0 < mean < 1.12                                     # Table 1's last column: 1.005 - 1.016 at 18-29 orbitals
+
+
+def test_rank_hubbard_chain():
+    from oracle import oracle as orc
+    r = _ranks(orc.hubbard_h(14, 1.0, 4.0), 14)
+    assert r[0] == 14 and all(v == 1 for x, v in r.items() if x)   # U sum n n: rank n_sites; hops: rank 1
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["q12", "q24"])
+def test_plan_key_counts_against_paper_ranks(name):
+    from paper_2606_28952_b200 import bs
+    cfg = si.CONFIGS[name]
+    n = cfg.n_orb
+    h, g = si.integrals(n, cfg.seed_ints)
+    op = bs.bs_jw_molecular(h, g)
+    sec = bs.bs_sector_build(n, cfg.n_alpha, cfg.n_beta)
+    x, nk = bs.bs_plan_groups(op, sec)
+    r = _ranks(oracle_operator(name), n)
+    info = bs.bs_plan_info(op, sec)
+    assert info["fallback"] == 0 and info["groups"] == len(x)
+    ma = (1 << n) - 1
+    seen = set()
+    for xm, k in zip(x.tolist(), nk.tolist()):
+        assert xm in r and xm not in seen                        # every plan group is one group of the operator
+        seen.add(xm)
+        pa, pb = bin(xm & ma).count("1"), bin(xm >> n).count("1")
+        if pa and pb:
+            assert k == 1 == r[xm]                               # alpha-beta groups: the paper's rank, exactly
+        elif pa == 4 or pb == 4:
+            assert k == 1 == r[xm]                               # same-spin doubles: one key
+        elif pa + pb == 2:
+            assert k == n + 1 and r[xm] == 2                     # single excitations: n + 1 keys (single-bit sign flips)
+        else:
+            assert xm == 0 and k == 1 + n + math.comb(n, 2) and r[0] == n + 2
+    assert seen == {xm for xm in r if all(bin(p).count("1") // 2 <= min(c, n - c) for p, c in
+                                          (((xm & ma), cfg.n_alpha), ((xm >> n), cfg.n_beta)))}
