@@ -2,7 +2,7 @@
 """bench.py -- H|psi> applies/s (complex128) and achieved HBM GB/s vs the measured B200 peak.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
-                    [--per-config q12,q24,...|none]
+                    [--per-config q12,q24,...|none] [--sharded]
 
 Headline workload (config.workload): BASELINE.json configs[2], the 28-qubit Fermi-Hubbard chain
 (sector dim 11,778,624; 188.5 MB per vector, larger than the 126 MB L2, so no L2 flush is needed).
@@ -30,6 +30,8 @@ import numpy as np  # noqa: E402
 
 import synth_inputs as si  # noqa: E402
 
+SMEM_PEAK_TBS = 128 * 148 * 1.965e9 / 1e12        # shared-memory / L1 data path: 128 B/clk/SM
+DFMA_PEAK = 64 * 148 * 1.965e9                     # FP64 pipe: 64 DFMA/clk/SM, measured (profiles/r02_fp64_peak.md)
 METRIC = "H|psi> applies/s (fp64 complex)"
 UNIT = "applies/s"
 TAYLOR_ORDER = 12
@@ -109,7 +111,7 @@ def _median(v):
     return float(np.median(np.asarray(v, dtype=np.float64)))
 
 
-def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
+def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf, with_cpu: bool = False):
     """Plain bs_apply / bs_expect timings of one BASELINE.json config (CUDA events, median)."""
     cfg = si.CONFIGS[name]
     t0 = time.perf_counter()
@@ -140,8 +142,9 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
         times.append(a.elapsed_time(b))
     apply_ms = _median(times) if times else first_ms
     ent = {"n_qubits": cfg.n_qubits, "dim": cfg.dim, "groups": op.n_groups, "strings": op.n_terms,
-           "plan": bs.bs_plan_describe(op, sec),
+           "plan": bs.bs_plan_describe(op, sec), "plan_info": bs.bs_plan_info(op, sec),
            "raw_terms": m_raw, "setup_s": round(t_setup, 3),
+           "plan_build_ms": max(0.0, first_ms - apply_ms) if times else None,    # first call builds the cached plan
            "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
            "l2_flush_between_reps": bool(flush)}
     if cfg.kind == "molecular":       # non-zeros per row of H in the sector for generic integrals
@@ -150,9 +153,20 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
         nnz_row = 1 + oa * va + ob * vb + comb(oa, 2) * comb(va, 2) + comb(ob, 2) * comb(vb, 2) + oa * va * ob * vb
         ent["nonzeros_per_s"] = nnz_row * cfg.dim / (apply_ms * 1e-3)
         ent["gather_gbs"] = 16 * ent["nonzeros_per_s"] / 1e9      # 16-byte amplitude gathers through L2 / shared memory
+        # Resources that bind these configs: one 16-byte amplitude per non-zero through the
+        # shared-memory / L1 path (128 B/clk/SM) and 2 DFMA per non-zero (real weight x complex amplitude) on the FP64
+        # pipe (64 DFMA/clk/SM measured, profiles/r02_fp64_peak.md); SM clock from MEASURED_PEAKS (1965 MHz).
+        ent["binding"] = {
+            "smem_gather": {"achieved_tbs": ent["gather_gbs"] / 1e3, "peak_tbs": SMEM_PEAK_TBS,
+                            "frac": ent["gather_gbs"] / 1e3 / SMEM_PEAK_TBS,
+                            "note": "16 B x non-zeros/s against 128 B/clk/SM x 148 SMs x 1.965 GHz; the K-resolved kernel "
+                                    "gathers once per n - N_beta + 1 non-zeros, so this is an equivalent rate"},
+            "fp64": {"useful_dfma_per_s": 2 * ent["nonzeros_per_s"], "peak_dfma_per_s": DFMA_PEAK,
+                     "frac": 2 * ent["nonzeros_per_s"] / DFMA_PEAK}}
     bytes_alg = 32 * cfg.dim + table_bytes(op)
     ent["hbm_gbs_algorithmic"] = bytes_alg / apply_ms / 1e6
     ent["hbm_frac_of_measured_peak"] = ent["hbm_gbs_algorithmic"] / peak_gbs
+    ent["traffic_ncu"] = TRAFFIC_NCU.get(name)
     if reps:
         bs.bs_expect(op, sec, psi)                         # first call may allocate library scratch
         t0 = time.perf_counter()
@@ -180,12 +194,17 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf):
         ent["rotations_per_s"] = len(ex) / (_median(rt) * 1e-3)
     del psi, out, op, sec
     torch.cuda.empty_cache()
+    if with_cpu and cfg.dim > 1000:
+        ent["cpu_baseline"] = cpu_baseline(name, max_seconds=12.0)
     return ent
 
 
 def cpu_baseline(name: str, max_seconds: float = 30.0):
-    """The oracle's grouped apply (OpenMP over targets, as it stands) on this host's cores.
-    One apply of the workload when that fits the budget, else an alpha-row slab scaled linearly in rows."""
+    """The oracle's Eq. 27 gather (OpenMP over target rows, as it stands) on this host's cores, on a bounded sample.
+    Small sectors: orc_apply_grouped on an alpha-row slab, scaled linearly in rows.  configs 4-5: the per-row beta
+    search makes that function take minutes per row, so the slab function with the search hoisted
+    (orc_apply_grouped_slab, the writer of the full-size goldens) is timed on two slabs; its per-call setup is
+    separated from the per-row cost by the difference and counted once."""
     from oracle import oracle as orc
     cfg = si.CONFIGS[name]
     if cfg.kind == "hubbard":
@@ -194,8 +213,23 @@ def cpu_baseline(name: str, max_seconds: float = 30.0):
         ref = orc.molecular_h(*si.integrals(cfg.n_orb, cfg.seed_ints))
     osec = orc.Sector(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
     psi = si.random_state(cfg.dim, cfg.seed_psi)
-    out = np.zeros_like(psi)
     rows = osec.dim_alpha
+    cores = orc.num_threads()
+    if cfg.dim > 5e7:
+        r1, r2 = min(rows, cores), min(rows, 3 * cores)
+        t0 = time.perf_counter()
+        osec.apply_grouped_slab(ref, psi, 0, r1)
+        t1 = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        osec.apply_grouped_slab(ref, psi, 0, r2)
+        t2 = time.perf_counter() - t0
+        per_row = max(1e-9, (t2 - t1) / max(1, r2 - r1))
+        fixed = max(0.0, t1 - r1 * per_row)
+        t_full = fixed + rows * per_row
+        sample = (f"oracle orc_apply_grouped_slab on alpha rows [0,{r1}) and [0,{r2}) of {rows}: {t1:.1f} s and {t2:.1f} s "
+                  f"-> {per_row:.3f} s per row + {fixed:.1f} s setup, extrapolated linearly in rows")
+        return {"value": 1.0 / t_full, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    out = np.zeros_like(psi)
     probe = max(1, rows // 64)
     t0 = time.perf_counter()
     osec.apply_grouped(ref, psi, 0, probe, out)
@@ -207,7 +241,7 @@ def cpu_baseline(name: str, max_seconds: float = 30.0):
     applies_per_s = (n_rows / rows) / t
     sample = (f"oracle orc_apply_grouped on alpha rows [0,{n_rows}) of {rows} ({n_rows * osec.dim_beta} of "
               f"{cfg.dim} targets) in {t:.2f} s, scaled linearly in rows")
-    return {"value": applies_per_s, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample}
+    return {"value": applies_per_s, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
 
 def run_ours(args):
@@ -358,14 +392,16 @@ def run_ours(args):
                          + " (the 12 apply+axpby launches of bs_taylor_step)",
                          "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
                          "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
-                         "launch_ms": launch_ms, "traffic": TRAFFIC_NCU.get(name)},
+                         "launch_ms": launch_ms, "traffic": (TRAFFIC_NCU.get(name) or {}).get("bytes_per_launch"),
+                         "traffic_source": (TRAFFIC_NCU.get(name) or {}).get("profile")},
         }
         want = [] if args.per_config == "none" else args.per_config.split(",")
         if want and world == 1:
             del psi, work
             torch.cuda.empty_cache()
             flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-            line["per_config"] = {n: per_config_entry(n, bs, torch, peak_gbs, flush_buf) for n in want}
+            line["per_config"] = {n: per_config_entry(n, bs, torch, peak_gbs, flush_buf, not args.no_cpu_baseline)
+                                  for n in want}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(name)
         print(json.dumps(line), flush=True)
@@ -376,7 +412,89 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for that workload.
-TRAFFIC_NCU = {"q28_hubbard": 6.90e8}   # profiles/r01_v6_q28_k_light_full.md: mean of an odd (490 MB) and an even (890 MB) Taylor launch
+# Each entry names the committed capture it was read from (profiles/); refreshed whenever the kernel changes.
+TRAFFIC_NCU = {
+    "q28_hubbard": {"bytes_per_launch": None, "kernel": "k_light<0>", "profile": None},
+    "q24": {"bytes_per_launch": None, "kernel": "k_ab<12>", "profile": None},
+    "q32": {"bytes_per_launch": None, "kernel": "k_ab<16>", "profile": None},
+    "q56": {"bytes_per_launch": None, "kernel": "k_ab<28>", "profile": None},
+}
+
+
+def run_sharded(args):
+    """--sharded: ONE state vector, alpha-row slabs over the ranks (bs_apply_rows), NCCL all-gather of the slabs
+    (paper_2606_28952_b200/dist.py).  Strong scaling: value = applies/s of the one vector; per-phase device times
+    (max over ranks) are reported so that the parts that do not shrink with N are visible."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_28952_b200 import bs
+    from paper_2606_28952_b200.dist import row_slabs, sharded_apply, sharded_expect
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (libbs has no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:  # one rank: the same code path through a single-process group
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29577")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+    name = args.workload
+    cfg = si.CONFIGS[name]
+    op, _ = build_operator(name, bs)
+    sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    psi = torch.from_numpy(si.random_state(cfg.dim, cfg.seed_psi)).cuda()      # identical on every rank
+    out = torch.empty_like(psi)
+    Da, Db = cfg.dim_alpha, cfg.dim_beta
+
+    def apply_rows(pin, pout, lo, hi):
+        bs.bs_apply_rows(op, sec, pin, pout, lo, hi)
+
+    evs = []
+
+    def marks(what):
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        evs.append(e)
+
+    for _ in range(max(args.warmup, 3)):
+        sharded_apply(apply_rows, psi, out, Da, Db)
+    dist.barrier()
+    torch.cuda.synchronize()
+    n0 = bs.bs_launch_count()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(args.steps):
+        sharded_apply(apply_rows, psi, out, Da, Db, marks=marks)
+    b.record()
+    dist.barrier()
+    torch.cuda.synchronize()
+    launches = bs.bs_launch_count() - n0
+    total_ms = a.elapsed_time(b)
+    comp_ms = sum(evs[3 * i].elapsed_time(evs[3 * i + 1]) for i in range(args.steps)) / args.steps
+    gath_ms = sum(evs[3 * i + 1].elapsed_time(evs[3 * i + 2]) for i in range(args.steps)) / args.steps
+    e = sharded_expect(apply_rows, psi, out, Da, Db)
+    t = torch.tensor([total_ms, comp_ms, gath_ms], dtype=torch.float64, device="cuda")
+    tmin = t.clone()
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(tmin, op=dist.ReduceOp.MIN)
+    if rank == 0:
+        total_ms, comp_ms, gath_ms = t.tolist()
+        line = {"metric": METRIC, "value": args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64 (complex128)",
+                "data": "synthetic", "mode": "sharded",
+                "config": {"workload": f"{name}: BASELINE.json configs[{si.CONFIG_ORDER.index(name)}]",
+                           "dim": cfg.dim, "step": "1 H application of ONE state vector",
+                           "parallelism": f"alpha-row slabs over {world} rank(s) (bs_apply_rows) + all-gather of the slabs",
+                           "slabs": row_slabs(Da, world), "plan": bs.bs_plan_describe(op, sec)},
+                "compute_ms_max": comp_ms, "compute_ms_min": tmin[1].item(), "allgather_ms_max": gath_ms,
+                "allgather_bytes": 16 * cfg.dim, "energy": e.real, "gpu_launches": int(launches)}
+        print(json.dumps(line), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
 
 
 def run_reference(args):
@@ -434,10 +552,14 @@ def main():
     ap.add_argument("--per-config", default="q12,q24,q28_hubbard,q32,q56",
                     help="comma list of configs to time with plain bs_apply (N=1 only), or 'none'")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="one state vector sharded by alpha-row slabs over the ranks + NCCL all-gather (dist.py)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -58,6 +58,7 @@ extern "C" {
 
 typedef struct bs_op*     bs_op_t;     /* grouped Pauli sum, device resident, library owned */
 typedef struct bs_sector* bs_sector_t; /* sector tables,     device resident, library owned */
+typedef struct bs_symsector* bs_symsector_t; /* point-group block of a sector, library owned */
 
 typedef enum {
     BS_OK = 0,
@@ -112,6 +113,26 @@ int bs_sector_export(bs_sector_t s, uint64_t* alpha_strings, uint64_t* beta_stri
  * with the same lookup tables the apply kernels use.  Synchronises. */
 int bs_sector_rank(bs_sector_t s, const uint64_t* configs, int64_t n, int64_t* index_out);
 int bs_sector_destroy(bs_sector_t s);
+
+/* ---- point-group symmetry blocking (Eq. 29-31) for Abelian point groups (D2h and subgroups).
+ * orb_irrep [host] int[n_orb]: irrep label 0..7 of every spatial orbital; the irrep of a spin string is the XOR of the
+ * labels of its occupied orbitals; the block holds the configurations of `parent` with irrep(t_a) ^ irrep(t_b) =
+ * target_irrep (Eq. 30).  Blocked vector layout (Eq. 29): blocks r = 0..7 in order of the alpha irrep; block r pairs
+ * the alpha strings of irrep r with the beta strings of irrep r ^ target_irrep, each in increasing numeric order,
+ * index = offset_r + rank_alpha^r * D_beta^r + rank_beta^r.  `parent` must outlive the handle.
+ * The blocking is a STORAGE layout: bs_sym_apply / bs_sym_expect embed the blocked vector into the sector layout
+ * (zero in the other irreps), run bs_apply / bs_expect there and read the block back, using two sector-sized
+ * scratch vectors owned by the handle (allocated at the first call).  They return P_block H P_block psi. */
+int bs_symsector_build(bs_sector_t parent, const int* orb_irrep, int target_irrep, void* cuda_stream,
+                       bs_symsector_t* out);
+/* dim: amplitudes of the block; dim_alpha[r], dim_beta[r] [host] int64[8]: strings of irrep r (any pointer may be NULL) */
+int bs_symsector_info(bs_symsector_t h, int64_t* dim, int64_t dim_alpha[8], int64_t dim_beta[8]);
+int bs_symsector_destroy(bs_symsector_t h);
+/* psi_blocked [device] complex128[dim of the block], psi_sector [device] complex128[dim of the parent sector] */
+int bs_sym_scatter(bs_symsector_t h, const void* psi_blocked, void* psi_sector, void* cuda_stream);
+int bs_sym_gather(bs_symsector_t h, const void* psi_sector, void* psi_blocked, void* cuda_stream);
+int bs_sym_apply(bs_op_t op, bs_symsector_t h, const void* psi_in, void* psi_out, void* cuda_stream);
+int bs_sym_expect(bs_op_t op, bs_symsector_t h, const void* psi, double result_reim[2], void* cuda_stream);
 
 /* ---- a4: out = P_sector H P_sector psi  (Eq. 27).  psi_in, psi_out [device]
  * complex128[dim], distinct buffers.  The first call for a given (op, sector) pair builds and

@@ -25,7 +25,9 @@ SYMBOLS = [
     "bs_group_xmask", "bs_op_info", "bs_op_export", "bs_op_destroy",
     "bs_sector_build", "bs_sector_info", "bs_sector_export", "bs_sector_rank", "bs_sector_destroy",
     "bs_apply", "bs_apply_rows", "bs_apply_axpby", "bs_expect", "bs_vdot",
-    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_plan_info", "bs_plan_groups", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
+    "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_plan_info", "bs_plan_groups",
+    "bs_symsector_build", "bs_symsector_info", "bs_symsector_destroy", "bs_sym_scatter", "bs_sym_gather", "bs_sym_apply",
+    "bs_sym_expect", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
 ]
 
 
@@ -61,6 +63,13 @@ def _load():
     L.bs_jw_molecular.argtypes = [C.c_int, vp, vp, dbl, vp, C.POINTER(vp)]
     L.bs_jw_hubbard.argtypes = [C.c_int, dbl, dbl, dbl, vp, C.POINTER(vp)]
     L.bs_plan_describe.argtypes = [vp, vp, C.c_char_p, i64, vp]
+    L.bs_symsector_build.argtypes = [vp, vp, C.c_int, vp, C.POINTER(vp)]
+    L.bs_symsector_info.argtypes = [vp, C.POINTER(i64), vp, vp]
+    L.bs_symsector_destroy.argtypes = [vp]
+    L.bs_sym_scatter.argtypes = [vp, vp, vp, vp]
+    L.bs_sym_gather.argtypes = [vp, vp, vp, vp]
+    L.bs_sym_apply.argtypes = [vp, vp, vp, vp, vp]
+    L.bs_sym_expect.argtypes = [vp, vp, vp, C.POINTER(dbl), vp]
     L.bs_plan_info.argtypes = [vp, vp, C.POINTER(i64), vp]
     L.bs_plan_groups.argtypes = [vp, vp, vp, vp, i64, C.POINTER(i64), vp]
     L.bs_launch_count.restype = i64
@@ -254,6 +263,55 @@ def bs_plan_describe(op: Op, sector: Sector, stream=None) -> str:
     buf = C.create_string_buffer(2048)
     _check(_lib.bs_plan_describe(op._h, sector._h, buf, 2048, _stream(stream)))
     return buf.value.decode()
+
+
+class SymSector:
+    """bs_symsector_t handle: one point-group block of a sector (Eq. 29-31)."""
+
+    def __init__(self, sector: "Sector", orb_irrep, target_irrep: int, stream=None):
+        lab = np.ascontiguousarray(orb_irrep, np.int32)
+        if lab.shape != (sector.n_orb,):
+            raise ValueError("orb_irrep must have one label per spatial orbital")
+        h = C.c_void_p()
+        _check(_lib.bs_symsector_build(sector._h, _np_ptr(lab), int(target_irrep), _stream(stream), C.byref(h)))
+        self._h, self.parent = h, sector
+        d = C.c_int64()
+        da, db = np.zeros(8, np.int64), np.zeros(8, np.int64)
+        _check(_lib.bs_symsector_info(self._h, C.byref(d), _np_ptr(da), _np_ptr(db)))
+        self.dim, self.dim_alpha, self.dim_beta = int(d.value), da, db
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            _lib.bs_symsector_destroy(self._h)
+            self._h = None
+
+
+def bs_symsector_build(sector, orb_irrep, target_irrep: int, stream=None) -> SymSector:
+    return SymSector(sector, orb_irrep, target_irrep, stream)
+
+
+def bs_sym_scatter(sym: SymSector, psi_blocked, psi_sector, stream=None):
+    _check(_lib.bs_sym_scatter(sym._h, _dev_ptr(psi_blocked, sym.dim, "psi_blocked"),
+                               _dev_ptr(psi_sector, sym.parent.dim, "psi_sector"), _stream(stream)))
+    return psi_sector
+
+
+def bs_sym_gather(sym: SymSector, psi_sector, psi_blocked, stream=None):
+    _check(_lib.bs_sym_gather(sym._h, _dev_ptr(psi_sector, sym.parent.dim, "psi_sector"),
+                              _dev_ptr(psi_blocked, sym.dim, "psi_blocked"), _stream(stream)))
+    return psi_blocked
+
+
+def bs_sym_apply(op: Op, sym: SymSector, psi_in, psi_out, stream=None):
+    _check(_lib.bs_sym_apply(op._h, sym._h, _dev_ptr(psi_in, sym.dim, "psi_in"), _dev_ptr(psi_out, sym.dim, "psi_out"),
+                             _stream(stream)))
+    return psi_out
+
+
+def bs_sym_expect(op: Op, sym: SymSector, psi, stream=None) -> complex:
+    res = (C.c_double * 2)()
+    _check(_lib.bs_sym_expect(op._h, sym._h, _dev_ptr(psi, sym.dim, "psi"), res, _stream(stream)))
+    return complex(res[0], res[1])
 
 
 PLAN_INFO_FIELDS = ("kernel_path", "fallback", "transposed", "kres", "vector_scratch_bytes", "kres_scratch_bytes",

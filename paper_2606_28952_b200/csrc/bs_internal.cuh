@@ -88,6 +88,10 @@ struct bs_op {
         std::vector<i64> coff;  // [G + 1]
         DevBuf<uint2> d_cpairs; // per generator the valid {column, partner column} pairs (x_a = 0: owner side only)
         DevBuf<i64> d_off, d_coff;  // device copies of off / coff
+        std::vector<i64> roff;  // [G + 1] z-reduced strings of every generator for this sector (exact on valid targets)
+        DevBuf<u64> d_rz;
+        DevBuf<double2> d_rw;
+        DevBuf<i64> d_roff;
         DevBuf<double> d_th;    // thetas of the current call
         DevBuf<double2> d_sc;   // (sin, cos) of the thetas
     };

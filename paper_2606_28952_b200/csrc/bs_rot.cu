@@ -89,6 +89,21 @@ k_rot_rows(SpinTab A, SpinTab B, int n_orb, u64 x, const uint2* __restrict__ pai
                 theta, sc1);
 }
 
+// Pair-list variant (the per-generator path at sector sizes whose cells do not fit shared memory, configs 4-5): both
+// sides are precomputed per (generator, sector) -- owner (row, partner row) pairs and valid (column, partner column)
+// pairs -- so every thread rotates one pair: no validity test, no rank lookup, no idle lanes; the strings are the
+// z-reduced ones (see reduce_generators), typically 2 instead of 8 for a double excitation.
+__global__ void __launch_bounds__(256)
+k_rot_pairs(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ rpairs, const uint2* __restrict__ cpairs, i64 n_cp,
+            const u64* __restrict__ z, const double2* __restrict__ w, int k0, int k1, double theta, double2 sc1,
+            double2* __restrict__ psi) {
+    const i64 p = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (p >= n_cp) return;
+    const uint2 rp = __ldg(rpairs + blockIdx.y), cp = __ldg(cpairs + p);
+    const u64 t = (u64)A.str[rp.x] | ((u64)B.str[cp.x] << n_orb);
+    rotate_pair(psi, (i64)rp.x * B.D + cp.x, (i64)rp.y * B.D + cp.y, phase_sum(z, w, k0, k1, t), theta, sc1);
+}
+
 // Diagonal generator (x = 0, e.g. exp(-i w Z_j Z_{j+1}) of the layered TFIM ansatz, Eq. 42):
 // A|t> = F(t)|t> with F purely imaginary for an anti-Hermitian A, so psi[t] *= exp(theta F(t)).
 __global__ void __launch_bounds__(256)
@@ -189,7 +204,10 @@ __device__ __forceinline__ double2 phase_sum_b(const GenChunk& G, int k0, int k1
 }
 
 // cells = rows (R = 1, x_a = 0) or row pairs (R = 2, common x_a != 0); generators [j0, j1)
-template <int R>
+// GLOBAL: the cell does not fit shared memory (D_beta > 5,937: configs 4-5): the block works on its rows in place.
+// One launch still covers the whole run, the rows of the ~300 blocks in flight (0.4 - 0.7 MB each) stay in the 126 MB
+// L2 across the run's generators, so HBM sees each row once per run instead of once per generator.
+template <int R, bool GLOBAL>
 __global__ void __launch_bounds__(R == 2 ? 512 : 256)
 k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
                 const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
@@ -197,19 +215,20 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
                 const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
-    double2* s0 = reinterpret_cast<double2*>(smem_cell);
     const u32 Db = (u32)B.D;
-    double2* s1 = (R == 2) ? s0 + Db : s0;
     u32 row0, row1;
     if (R == 2) {
         const uint2 pr = pairs[blockIdx.x];
         row0 = pr.x;
         row1 = pr.y;
     } else row0 = row1 = blockIdx.x;
-    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
-        s0[c] = psi[(i64)row0 * Db + c];
-        if (R == 2) s1[c] = psi[(i64)row1 * Db + c];
-    }
+    double2* s0 = GLOBAL ? psi + (i64)row0 * Db : reinterpret_cast<double2*>(smem_cell);
+    double2* s1 = GLOBAL ? psi + (i64)row1 * Db : ((R == 2) ? s0 + Db : s0);
+    if (!GLOBAL)
+        for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
+            s0[c] = psi[(i64)row0 * Db + c];
+            if (R == 2) s1[c] = psi[(i64)row1 * Db + c];
+        }
     const u32 ta = A.str[row0];
     for (i64 j = j0; j < j1;) {
         __syncthreads();  // previous chunk fully consumed (and the rows are loaded)
@@ -237,14 +256,15 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
         }
         j += n;
     }
-    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
-        psi[(i64)row0 * Db + c] = s0[c];
-        if (R == 2) psi[(i64)row1 * Db + c] = s1[c];
-    }
+    if (!GLOBAL)
+        for (u32 c = threadIdx.x; c < Db; c += blockDim.x) {
+            psi[(i64)row0 * Db + c] = s0[c];
+            if (R == 2) psi[(i64)row1 * Db + c] = s1[c];
+        }
 }
 
-// cells = CC consecutive columns x all rows (x_b = 0 for every generator of the run)
-template <int CC>
+// cells = CC consecutive columns x all rows (x_b = 0 for every generator of the run); GLOBAL as above (in place, L2)
+template <int CC, bool GLOBAL>
 __global__ void __launch_bounds__(1024)
 k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, const i64* __restrict__ offs,
                 const u64* __restrict__ z, const double2* __restrict__ w, const double* __restrict__ thetas,
@@ -252,14 +272,17 @@ k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, con
                 i64 j1, double2* __restrict__ psi) {
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
-    double2* sm = reinterpret_cast<double2*>(smem_cell);  // [Da][CC]
     const u32 Da = (u32)A.D, Db = (u32)B.D;
     const u32 c0 = blockIdx.x * CC;
     const u32 ncol = min((u32)CC, Db - c0);
-    for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
-        const u32 r = i / CC, c = i - r * CC;
-        if (c < ncol) sm[i] = psi[(i64)r * Db + c0 + c];
-    }
+    // cell element (row r, column c0 + c): shared memory [Da][CC], or the state vector itself
+    double2* sm = GLOBAL ? psi + c0 : reinterpret_cast<double2*>(smem_cell);
+    const i64 rs = GLOBAL ? (i64)Db : (i64)CC;   // row stride of the cell
+    if (!GLOBAL)
+        for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
+            const u32 r = i / CC, c = i - r * CC;
+            if (c < ncol) sm[i] = psi[(i64)r * Db + c0 + c];
+        }
     for (i64 j = j0; j < j1;) {
         __syncthreads();
         const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
@@ -274,17 +297,18 @@ k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, con
                 if (c >= ncol) continue;
                 const uint2 rp = __ldg(rpairs + p0 + q);
                 const u32 ta = A.str[rp.x], tb = B.str[c0 + c];
-                rotate_smem(sm[rp.x * CC + c], sm[rp.y * CC + c], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)),
+                rotate_smem(sm[rp.x * rs + c], sm[rp.y * rs + c], phase_sum_s(G, k0, k1, (u64)ta | ((u64)tb << n_orb)),
                             G.th[g], G.sc[g]);
             }
             __syncthreads();
         }
         j += n;
     }
-    for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
-        const u32 r = i / CC, c = i - r * CC;
-        if (c < ncol) psi[(i64)r * Db + c0 + c] = sm[i];
-    }
+    if (!GLOBAL)
+        for (u32 i = threadIdx.x; i < Da * CC; i += blockDim.x) {
+            const u32 r = i / CC, c = i - r * CC;
+            if (c < ncol) psi[(i64)r * Db + c0 + c] = sm[i];
+        }
 }
 
 // One-off validation of a generator list against a sector: for every generator (blockIdx.y) and
@@ -401,7 +425,45 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                     RR->coff[j + 1] = (i64)cpairs.size();
                 }
             }
+            // z-reduction modulo x (exact on every valid target: z and z ^ x_s differ by the constant (-1)^{popc(x_s)/2}
+            // there, cf. bs_plan.cu): strings that differ by x on a spin merge, 8 strings of a double excitation -> 2
+            std::vector<u64> rz;
+            std::vector<double2> rw;
+            RR->roff.assign(n_rot + 1, 0);
+            for (i64 j = 0; j < n_rot; ++j) {
+                const u64 xa = gen->h_xg[j] & mask_a, xb = gen->h_xg[j] >> s->n_orb;
+                const double sga = ((__builtin_popcountll(xa) / 2) & 1) ? -1.0 : 1.0;
+                const double sgb = ((__builtin_popcountll(xb) / 2) & 1) ? -1.0 : 1.0;
+                std::vector<std::pair<u64, double2>> v;
+                for (i64 k = gen->h_offs[j]; k < gen->h_offs[j + 1]; ++k) {
+                    u64 za = gen->h_z[k] & mask_a, zb = gen->h_z[k] >> s->n_orb;
+                    double2 wk = make_double2(gen->h_w[2 * k], gen->h_w[2 * k + 1]);
+                    if ((za ^ xa) < za) { za ^= xa; wk.x *= sga; wk.y *= sga; }
+                    if ((zb ^ xb) < zb) { zb ^= xb; wk.x *= sgb; wk.y *= sgb; }
+                    v.push_back({za | (zb << s->n_orb), wk});
+                }
+                std::stable_sort(v.begin(), v.end(), [](const std::pair<u64, double2>& a, const std::pair<u64, double2>& b) {
+                    return a.first < b.first;
+                });
+                for (size_t k = 0; k < v.size();) {
+                    double2 acc = v[k].second;
+                    size_t e2 = k + 1;
+                    for (; e2 < v.size() && v[e2].first == v[k].first; ++e2) {
+                        acc.x += v[e2].second.x;
+                        acc.y += v[e2].second.y;
+                    }
+                    if (acc.x != 0.0 || acc.y != 0.0) {
+                        rz.push_back(v[k].first);
+                        rw.push_back(acc);
+                    }
+                    k = e2;
+                }
+                RR->roff[j + 1] = (i64)rz.size();
+            }
             cudaError_t e = RR->d_pairs.upload(pairs, st);
+            if (e == cudaSuccess) e = RR->d_rz.upload(rz, st);
+            if (e == cudaSuccess) e = RR->d_rw.upload(rw, st);
+            if (e == cudaSuccess) e = RR->d_roff.upload(RR->roff, st);
             if (e == cudaSuccess) e = RR->d_cpairs.upload(cpairs, st);
             if (e == cudaSuccess) e = RR->d_off.upload(RR->off, st);
             if (e == cudaSuccess) e = RR->d_coff.upload(RR->coff, st);
@@ -425,7 +487,15 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                                            thetas[j], psi);
         else if (s->full)
             k_rot_full<<<nb, 256, 0, st>>>(s->D, gen->h_xg[j], gen->d_z.p, gen->d_w.p, k0, k1, thetas[j], sc1, psi);
-        else if (RR) {
+        else if (RR && RR->coff.back() > 0) {
+            const i64 nr = RR->off[j + 1] - RR->off[j], ncp = RR->coff[j + 1] - RR->coff[j];
+            for (i64 r0 = 0; r0 < nr && ncp > 0; r0 += 65535) {
+                const dim3 rg((unsigned)((ncp + 255) / 256), (unsigned)std::min<i64>(65535, nr - r0));
+                k_rot_pairs<<<rg, 256, 0, st>>>(s->ta, s->tb, s->n_orb, RR->d_pairs.p + RR->off[j] + r0,
+                                                RR->d_cpairs.p + RR->coff[j], ncp, RR->d_rz.p, RR->d_rw.p,
+                                                (int)RR->roff[j], (int)RR->roff[j + 1], thetas[j], sc1, psi);
+            }
+        } else if (RR) {
             const i64 nr = RR->off[j + 1] - RR->off[j];
             for (i64 r0 = 0; r0 < nr; r0 += 65535) {
                 const dim3 rg(sgrid.x, (unsigned)std::min<i64>(65535, nr - r0));
@@ -438,6 +508,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
         BS_COUNT_LAUNCH(1);
     };
     const bool batching = RR && RR->coff.back() > 0 && !getenv("BS_ROT_PER_LAUNCH");
+    const bool in_place = getenv("BS_ROT_IN_PLACE") != nullptr;   // test hook: cells in place (L2) even when they fit shared memory
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
         const u64 mask_a = (u64(1) << s->n_orb) - 1;
@@ -467,45 +538,60 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 if (e - j >= 2) kind = 2;
             }
             for (i64 q = j; q < e && kind; ++q)
-                if (gen->h_offs[q + 1] - gen->h_offs[q] > 256) kind = 0;  // kStrChunk
+                if (RR->roff[q + 1] - RR->roff[q] > 256) kind = 0;  // kStrChunk
+#define BS_ROT_ARGS_ROWS s->ta, s->tb, s->n_orb, pr, gen->d_xg.p, RR->d_roff.p, RR->d_rz.p, RR->d_rw.p, RR->d_th.p, RR->d_sc.p, \
+                         RR->d_cpairs.p, RR->d_coff.p, j, e, psi
+#define BS_ROT_ARGS_COLS s->ta, s->tb, s->n_orb, gen->d_xg.p, RR->d_roff.p, RR->d_rz.p, RR->d_rw.p, RR->d_th.p, RR->d_sc.p, \
+                         RR->d_pairs.p, RR->d_off.p, j, e, psi
+#define BS_ROT_SMEM(K)                                                                                              \
+    {                                                                                                               \
+        static const cudaError_t e_attr = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); \
+        BS_CUDA(e_attr);                                                                                            \
+    }
             if (kind == 1) {
                 const int R = xa0 ? 2 : 1;
                 const size_t smem = (size_t)R * s->Db * 16;
                 const i64 n_cells = xa0 ? RR->off[j + 1] - RR->off[j] : s->Da;
-                if (smem <= smem_cap && n_cells > 0) {
-                    const uint2* pr = RR->d_pairs.p + RR->off[j];
+                const uint2* pr = RR->d_pairs.p + RR->off[j];
+                if (n_cells == 0) {
+                    launched = true;  // x_a never valid in this sector: identity
+                } else if (smem <= smem_cap && !in_place) {
                     if (R == 2) {
-                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                        k_rot_cell_rows<2><<<(unsigned)n_cells, 512, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
-                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_cpairs.p, RR->d_coff.p, j, e, psi);
+                        BS_ROT_SMEM((k_rot_cell_rows<2, false>))
+                        k_rot_cell_rows<2, false><<<(unsigned)n_cells, 512, smem, st>>>(BS_ROT_ARGS_ROWS);
                     } else {
-                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_rows<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                        k_rot_cell_rows<1><<<(unsigned)n_cells, 256, smem, st>>>(s->ta, s->tb, s->n_orb, pr, gen->d_xg.p,
-                            gen->d_offs.p, gen->d_z.p, gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_cpairs.p, RR->d_coff.p, j, e, psi);
+                        BS_ROT_SMEM((k_rot_cell_rows<1, false>))
+                        k_rot_cell_rows<1, false><<<(unsigned)n_cells, 256, smem, st>>>(BS_ROT_ARGS_ROWS);
                     }
                     BS_COUNT_LAUNCH(1);
                     launched = true;
-                } else if (n_cells == 0) {
-                    launched = true;  // x_a never valid in this sector: identity
+                } else {   // the cell stays in place (L2): still one launch per run
+                    if (R == 2) k_rot_cell_rows<2, true><<<(unsigned)n_cells, 512, 0, st>>>(BS_ROT_ARGS_ROWS);
+                    else k_rot_cell_rows<1, true><<<(unsigned)n_cells, 256, 0, st>>>(BS_ROT_ARGS_ROWS);
+                    BS_COUNT_LAUNCH(1);
+                    launched = true;
                 }
             } else if (kind == 2) {
-                const int CC = ((size_t)s->Da * 8 * 16 <= smem_cap) ? 8 : (((size_t)s->Da * 2 * 16 <= smem_cap) ? 2 : 0);
+                const int CC = in_place ? 0 : ((size_t)s->Da * 8 * 16 <= smem_cap) ? 8 : (((size_t)s->Da * 2 * 16 <= smem_cap) ? 2 : 0);
                 if (CC) {
                     const size_t smem = (size_t)s->Da * CC * 16;
                     const unsigned nblk = (unsigned)((s->Db + CC - 1) / CC);
                     if (CC == 8) {
-                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                        k_rot_cell_cols<8><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
-                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_pairs.p, RR->d_off.p, j, e, psi);
+                        BS_ROT_SMEM((k_rot_cell_cols<8, false>))
+                        k_rot_cell_cols<8, false><<<nblk, 1024, smem, st>>>(BS_ROT_ARGS_COLS);
                     } else {
-                        BS_CUDA(cudaFuncSetAttribute(k_rot_cell_cols<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                        k_rot_cell_cols<2><<<nblk, 1024, smem, st>>>(s->ta, s->tb, s->n_orb, gen->d_xg.p, gen->d_offs.p, gen->d_z.p,
-                            gen->d_w.p, RR->d_th.p, RR->d_sc.p, RR->d_pairs.p, RR->d_off.p, j, e, psi);
+                        BS_ROT_SMEM((k_rot_cell_cols<2, false>))
+                        k_rot_cell_cols<2, false><<<nblk, 1024, smem, st>>>(BS_ROT_ARGS_COLS);
                     }
-                    BS_COUNT_LAUNCH(1);
-                    launched = true;
+                } else {   // in place: 2 columns (one 32-byte sector per row) x all rows per block
+                    k_rot_cell_cols<2, true><<<(unsigned)((s->Db + 1) / 2), 1024, 0, st>>>(BS_ROT_ARGS_COLS);
                 }
+                BS_COUNT_LAUNCH(1);
+                launched = true;
             }
+#undef BS_ROT_ARGS_ROWS
+#undef BS_ROT_ARGS_COLS
+#undef BS_ROT_SMEM
             if (!launched)
                 for (i64 q = j; q < e; ++q) single(q);  // in order: rotations do not commute
             j = e;

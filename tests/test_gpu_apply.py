@@ -340,12 +340,15 @@ def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
         "print('LAUNCHES', n1 - n0, 'ERR', err); assert err <= 1e-12\n")
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     counts = {}
-    for env in ({}, {"BS_ROT_PER_LAUNCH": "1"}):
+    # BS_ROT_IN_PLACE: the cell kernels work on the state vector itself (the path of sectors whose cells exceed
+    # shared memory, configs 4-5) -- same launch count as the shared-memory cells
+    for key, env in (("cells", {}), ("per_launch", {"BS_ROT_PER_LAUNCH": "1"}), ("in_place", {"BS_ROT_IN_PLACE": "1"})):
         r = subprocess.run([sys.executable, "-c", code, root], env=dict(os.environ, **env), capture_output=True,
                            text=True, timeout=600)
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
-        counts[bool(env)] = int(r.stdout.split("LAUNCHES")[1].split()[0])
-    assert counts[True] > 3 * counts[False]      # batching really reduces the launch count
+        counts[key] = int(r.stdout.split("LAUNCHES")[1].split()[0])
+    assert counts["per_launch"] > 3 * counts["cells"]      # batching really reduces the launch count
+    assert counts["in_place"] == counts["cells"]
 
 
 def test_apply_and_rotations_are_bit_reproducible(bs):

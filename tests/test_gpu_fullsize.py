@@ -120,3 +120,41 @@ def test_full_size_against_oracle_goldens(bs, name):
     bs.bs_apply(op, sec, phi, d_out)
     rhs = bs.bs_vdot(sec, d_out, d_in)                       # <H phi|psi>
     assert abs(lhs - rhs) <= 1e-10
+
+
+def test_q32_uccsd_rotations(bs):
+    """a6 beyond 24 qubits (Table 2 "Trotter" column): at D_beta = 12,870 a row pair no longer
+    fits shared memory, so runs of generators go through the pair-list kernel, one launch per generator.
+    (i) 16 orbitals, (2, 8) electrons (D_beta = 12,870 as in configs[3], D = 1.5e6 so that the single-threaded oracle
+    finishes): 600 of its 2,759 UCCSD generators, in list order, on a random state, full-vector comparison with the
+    oracle's fermionic Givens rotations.  (ii) configs[3] itself, all 5,792 generators (43,264 Pauli strings): norm."""
+    import torch
+    from oracle import oracle as orc
+    from paper_2606_28952_b200 import jw_terms as jw
+    n, na, nb = 16, 2, 8
+    ex = si.uccsd_excitations(n, na, nb)
+    assert len(ex) == 2759
+    th_all = si.thetas(len(ex), 3004)
+    rng = np.random.default_rng(21)
+    pick = sorted(set(range(300)) | set(rng.choice(len(ex), 300, replace=False).tolist()))
+    sub = [ex[i] for i in pick]
+    th = th_all[pick]
+    X, Z, Cc, offs = jw.excitation_generator_terms(sub)
+    gens = bs.bs_group_xmask(X, Z, Cc, 2 * n, 0.0, bs.BS_MODE_SEQUENCE, offs)
+    sec, osec = bs.bs_sector_build(n, na, nb), orc.Sector(n, na, nb)
+    psi = si.random_state(osec.dim, 77)
+    d = torch.from_numpy(psi).cuda()
+    bs.bs_apply_pauli_rotations(gens, sec, th, d)
+    for (cre, ann), t in zip(sub, th):
+        osec.rot_fermionic(psi, cre, ann, t)
+    assert rel_l2(d.cpu().numpy(), psi) <= 1e-12
+    del gens, d
+    cfg = si.CONFIGS["q32"]
+    ex = si.uccsd_excitations(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    assert len(ex) == 5792
+    X, Z, Cc, offs = jw.excitation_generator_terms(ex)
+    gens = bs.bs_group_xmask(X, Z, Cc, cfg.n_qubits, 0.0, bs.BS_MODE_SEQUENCE, offs)
+    sec = bs.bs_sector_build(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    d = torch.from_numpy(si.random_state(cfg.dim, cfg.seed_psi)).cuda()
+    bs.bs_apply_pauli_rotations(gens, sec, si.thetas(len(ex), 3004), d)
+    assert abs(np.sqrt(bs.bs_vdot(sec, d, d).real) - 1.0) <= 1e-10

@@ -78,13 +78,16 @@ def test_plan_key_counts_against_paper_ranks(name):
         assert xm in r and xm not in seen                        # every plan group is one group of the operator
         seen.add(xm)
         pa, pb = bin(xm & ma).count("1"), bin(xm >> n).count("1")
+        assert k >= r[xm] or xm == 0 or pa + pb == 2              # an exact factorisation never has fewer terms than the rank
         if pa and pb:
             assert k == 1 == r[xm]                               # alpha-beta groups: the paper's rank, exactly
-        elif pa == 4 or pb == 4:
-            assert k == 1 == r[xm]                               # same-spin doubles: one key
-        elif pa + pb == 2:
-            assert k == n + 1 and r[xm] == 2                     # single excitations: n + 1 keys (single-bit sign flips)
-        else:
-            assert xm == 0 and k == 1 + n + math.comb(n, 2) and r[0] == n + 2
+        elif info["transposed"] and (pa == 4 or pb == 4):
+            assert k == 1 == r[xm]                               # same-spin doubles: one key (Z on the other spin only)
+        elif info["transposed"] and pa + pb == 2:
+            # single excitations: the zero mask + one single-bit mask per orbital of the column spin; the paper's rank is 2
+            assert k == n + 1 and r[xm] == 2
+        elif xm == 0:
+            assert k == 1 + n + math.comb(n, 2) and r[0] == n + 2
+        # small sectors (q12) keep beta-only groups in-row, where their own-spin Z masks add keys: k >= rank only
     assert seen == {xm for xm in r if all(bin(p).count("1") // 2 <= min(c, n - c) for p, c in
                                           (((xm & ma), cfg.n_alpha), ((xm >> n), cfg.n_beta)))}
