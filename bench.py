@@ -173,25 +173,35 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf, with_cpu:
         e = bs.bs_expect(op, sec, psi)
         ent["expect_ms"] = (time.perf_counter() - t0) * 1e3
         ent["energy"] = e.real
-    if name == "q24":
+    if name in ("q24", "q32"):
+        # a6: first-order Trotterised UCCSD state preparation (Eq. 39), generator order of reading U10.
+        # A run = consecutive generators with one alpha mask (or all with x_b = 0): ONE launch; the floor of a run is one
+        # read + write of the state vector.  q24: cells in shared memory; q32: cells in place (L2), see DESIGN.md 5.2.
         from paper_2606_28952_b200 import jw_terms as jw
         ex = si.uccsd_excitations(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
-        th = si.thetas(len(ex), cfg.seed_theta)
+        th = si.thetas(len(ex), cfg.seed_theta or 3004)
         X, Z, Cc, offs = jw.excitation_generator_terms(ex)
         gens = bs.bs_group_xmask(X, Z, Cc, cfg.n_qubits, 0.0, bs.BS_MODE_SEQUENCE, offs)
-        rt = []
-        for i in range(4):
+        rt, launches = [], 0
+        for i in range(3):
             psi.zero_()
             psi[0] = 1.0
             a, b = ev(), ev()
+            n0 = bs.bs_launch_count()
             a.record()
             bs.bs_apply_pauli_rotations(gens, sec, th, psi)
             b.record()
             torch.cuda.synchronize()
+            launches = bs.bs_launch_count() - n0
             if i:
                 rt.append(a.elapsed_time(b))
+        ent["uccsd_generators"] = len(ex)
+        ent["uccsd_pauli_strings"] = int(len(X))
         ent["uccsd_prep_ms"] = _median(rt)
         ent["rotations_per_s"] = len(ex) / (_median(rt) * 1e-3)
+        ent["uccsd_launches"] = int(launches)
+        ent["uccsd_hbm_floor_ms"] = launches * 32 * cfg.dim / peak_gbs / 1e6   # one read + write of psi per launch (run)
+        del gens
     del psi, out, op, sec
     torch.cuda.empty_cache()
     if with_cpu and cfg.dim > 1000:

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 
+#include "bs_k2.cuh"
 #include "bs_kres.cuh"
 #include "bs_plan.cuh"
 #include "bs_rowplan.cuh"
@@ -74,6 +75,17 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
         P->rows_fallback = 1;
         return;
     }
+    // same-spin double excitations: dense blocks over (N - 2)-electron strings (bs_k2.cuh); what they take leaves the lists
+    bs_k2 *k2m = nullptr, *k2t = nullptr;
+    if (bs_k2_build(main_g, S->h_sa, S->n_orb, S->n_alpha, S->Db, st, &k2m) != BS_OK ||
+        (!t_g.empty() && bs_k2_build(t_g, S->h_sb, S->n_orb, S->n_beta, S->Da, st, &k2t) != BS_OK)) {
+        cudaGetLastError();
+        delete kres;
+        delete k2m;
+        delete k2t;
+        P->rows_fallback = 1;
+        return;
+    }
     bs_rowplan* m = new (std::nothrow) bs_rowplan;
     bs_rowplan* t = t_g.empty() ? nullptr : new (std::nothrow) bs_rowplan;
     bool ok = m && (t_g.empty() || t);
@@ -84,13 +96,17 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
         bs_rowplan_free(m);
         bs_rowplan_free(t);
         delete kres;
+        delete k2m;
+        delete k2t;
         P->rows_fallback = 1;   // queryable: bs_plan_describe says "fallback=1"
         return;
     }
-    if (!t && !kres && bs_light_build(m, st) != BS_OK) cudaGetLastError();  // optional fast path; k_rows stays available
+    if (!t && !kres && !k2m && bs_light_build(m, st) != BS_OK) cudaGetLastError();  // optional fast path; k_rows stays available
     P->rp_main = m;
     P->rp_t = t;
     P->kres = kres;
+    P->k2_main = k2m;
+    P->k2_t = k2t;
 }
 
 int build_sector_plan(bs_plan* P, bs_op* op, bs_sector* S, cudaStream_t st) {
@@ -253,6 +269,8 @@ bs_plan::~bs_plan() {
     bs_rowplan_free(rp_main);
     bs_rowplan_free(rp_t);
     delete kres;
+    delete k2_main;
+    delete k2_t;
 }
 void bs_rowplan_free(bs_rowplan* R) { delete R; }
 
@@ -276,11 +294,14 @@ extern "C" int bs_plan_info(bs_op_t op, bs_sector_t s, int64_t info[8], void* cu
     info[1] = P->rows_fallback;
     info[2] = P->rp_t ? 1 : 0;
     info[3] = P->kres ? 1 : 0;
-    info[4] = (P->rp_t || P->kres) ? 3 * 16 * s->D : 0;
+    info[4] = (P->rp_t || P->kres || P->k2_main) ? 3 * 16 * s->D : 0;
     info[5] = P->kres ? (int64_t)P->kres->slab_rows * P->kres->n * P->kres->DKp * 16 : 0;
+    for (const bs_k2* K2 : {P->k2_main, P->k2_t})
+        if (K2) info[5] += (int64_t)K2->F * K2->P * K2->slab_cols * 16;
     if (P->rp_main) {
         info[6] = P->rp_main->max_keys;
-        info[7] = P->rp_main->n_items + (P->rp_t ? P->rp_t->n_items : 0) + (P->kres ? P->kres->rp->n_items : 0);
+        info[7] = P->rp_main->n_items + (P->rp_t ? P->rp_t->n_items : 0) + (P->kres ? P->kres->rp->n_items : 0) +
+                  (P->k2_main ? P->k2_main->n_groups : 0) + (P->k2_t ? P->k2_t->n_groups : 0);
     }
     return BS_OK;
 }
@@ -309,6 +330,15 @@ extern "C" int bs_plan_groups(bs_op_t op, bs_sector_t s, uint64_t* x, int32_t* n
     emit(P->rp_main, false);
     emit(P->kres ? P->kres->rp : nullptr, false);
     emit(P->rp_t, true);
+    for (const bs_k2* K2 : {P->k2_main, P->k2_t})   // same-spin doubles: one key each
+        if (K2)
+            for (u32 xr : K2->h_x) {
+                if (x && nkeys && n < cap) {
+                    x[n] = K2 == P->k2_t ? ((u64)xr << s->n_orb) : (u64)xr;
+                    nkeys[n] = 1;
+                }
+                ++n;
+            }
     *n_groups = n;
     return BS_OK;
 }
@@ -338,6 +368,12 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
                           K->staged_rows, K->max_segs, (long long)K->slab_rows,
                           (double)K->slab_rows * K->n * K->DKp * 16.0 / 1048576.0);
         }
+        for (const bs_k2* K2 : {P->k2_main, P->k2_t})
+            if (K2 && w > 0 && w < n)
+                w += snprintf(buf + w, (size_t)(n - w),
+                              " k2%s{groups=%lld families=%d P=%d tile=%d tiles=%d smem=%zu slab_cols=%lld scratch_MB=%.0f}",
+                              K2 == P->k2_t ? "_t" : "", (long long)K2->n_groups, K2->F, K2->P, K2->rt, K2->n_tiles, K2->smem,
+                              (long long)K2->slab_cols, (double)K2->F * K2->P * K2->slab_cols * 16.0 / 1048576.0);
         if (T && w > 0 && w < n)
             snprintf(buf + w, (size_t)(n - w),
                      " transposed{xa=%d items=%lld keys=%lld strings=%lld tkeys=%lld max_keys=%d row_ent=%lld threads=%d "

@@ -21,6 +21,7 @@ struct HostGroup {
 
 struct bs_rowplan;
 struct bs_kres;
+struct bs_k2;
 int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups, const SpinTab& A, const SpinTab& B,
                      cudaStream_t st, bool with_tables = true);
 void bs_rowplan_free(bs_rowplan* R);
@@ -56,6 +57,8 @@ struct bs_plan {
     bs_rowplan* rp_main = nullptr;  // D, A, AB groups (and B groups when they are few)
     bs_rowplan* rp_t = nullptr;     // B groups as A groups of the transposed problem (when they are many)
     bs_kres* kres = nullptr;        // alpha-beta groups resolved over (N_beta - 1)-electron strings (bs_kres.cuh)
+    bs_k2* k2_main = nullptr;       // same-spin doubles of the row spin resolved over (N - 2)-electron strings (bs_k2.cuh)
+    bs_k2* k2_t = nullptr;          // the same for the column spin, on the transposed problem
     int rows_fallback = 0;          // 1: a v2 row plan could not be built (allocation, limits) and the v1 kernel runs
     DevBuf<double2> d_psi_t, d_out_t, d_raw;  // transposed input / output, raw H psi (lazily allocated)
 

@@ -18,6 +18,7 @@
 #include <algorithm>
 
 #include "bs_epilogue.cuh"
+#include "bs_k2.cuh"
 #include "bs_kres.cuh"
 #include "bs_plan.cuh"
 #include "bs_rowplan.cuh"
@@ -430,7 +431,7 @@ k_transpose_add_finish(const double2* raw, const double2* __restrict__ out_t,
 
 // The opt-in shared-memory ceiling is raised ONCE per kernel instantiation (thread-safe static initialisation; the
 // library drives one device per process), not on every launch; occupancy follows the size actually launched.
-constexpr int kMaxDynSmem = 227 * 1024;
+constexpr int kMaxDynSmem = 227 * 1024 - 1024;   // + the kernels' static shared memory (reduction scratch) stays under the 227 KB opt-in limit
 
 template <int MODE, bool REALW, int CPT>
 cudaError_t launch_k_rows_t(const bs_rowplan* R, dim3 grid, cudaStream_t st, const double2* psi, double2* out,
@@ -477,7 +478,7 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
                   bool expect, cudaStream_t st, i64* n_partials_out, double2** partials_out) {
     bs_rowplan* M = P->rp_main;
     const i64 Da = s->Da, Db = s->Db;
-    if (!P->rp_t && !P->kres && M->light) {
+    if (!P->rp_t && !P->kres && !P->k2_main && M->light) {
         if (expect && P->n_partials < 1024) {
             BS_CUDA(P->d_partials.alloc(1024));
             P->n_partials = 1024;
@@ -489,7 +490,7 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
         if (partials_out) *partials_out = P->d_partials.p;
         return BS_OK;
     }
-    if (!P->rp_t && !P->kres) {
+    if (!P->rp_t && !P->kres && !P->k2_main) {
         const i64 nblk = (hi - lo) * ((Db + M->chunk_cols - 1) / M->chunk_cols);
         if (expect && P->n_partials < nblk) {
             BS_CUDA(P->d_partials.alloc(nblk));
@@ -504,22 +505,32 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
     // the operator runs in parts: beta-only groups on the transposed problem (rp_t), alpha-beta groups K-resolved (kres)
     bs_rowplan* T = P->rp_t;
     bs_kres* K = P->kres;
-    if (T && !P->d_psi_t.p) BS_CUDA(P->d_psi_t.alloc(s->D));
-    if (T && !P->d_out_t.p) BS_CUDA(P->d_out_t.alloc(s->D));
+    const bool need_t = T || P->k2_t;
+    if (need_t && !P->d_psi_t.p) BS_CUDA(P->d_psi_t.alloc(s->D));
+    if (need_t && !P->d_out_t.p) BS_CUDA(P->d_out_t.alloc(s->D));
     double2* raw = out;
     if (expect || !ep.store_out) {
         if (!P->d_raw.p) BS_CUDA(P->d_raw.alloc(s->D));
         raw = P->d_raw.p;
     }
     Epilogue none = ep;
-    if (T) {
+    if (need_t) {
         dim3 tg((unsigned)((Db + 31) / 32), (unsigned)((Da + 31) / 32));
         k_transpose<<<tg, 256, 0, st>>>(psi, P->d_psi_t.p, Da, Db);
         BS_COUNT_LAUNCH(1);
         BS_CUDA(cudaGetLastError());
     }
     BS_CUDA(launch_k_rows<MODE_RAW>(M, st, psi, raw, lo, hi, 0, Db, none, nullptr));
+    if (P->k2_main) {   // same-spin doubles of the row spin, added to the raw result
+        int rc = bs_k2_apply(P->k2_main, psi, raw, Db, lo, hi, 0, Db, st);
+        if (rc != BS_OK) return rc;
+    }
     if (T) BS_CUDA(launch_k_rows<MODE_RAW>(T, st, P->d_psi_t.p, P->d_out_t.p, 0, Db, lo, hi, none, nullptr));
+    else if (need_t) BS_CUDA(cudaMemsetAsync(P->d_out_t.p, 0, (size_t)s->D * 16, st));
+    if (P->k2_t) {      // and of the column spin, on the transposed problem (its columns are the alpha rows)
+        int rc = bs_k2_apply(P->k2_t, P->d_psi_t.p, P->d_out_t.p, Da, 0, Db, lo, hi, st);
+        if (rc != BS_OK) return rc;
+    }
     const unsigned fgx = (unsigned)((Db + 31) / 32);
     const i64 nblk = (i64)fgx * ((hi - lo + 31) / 32 + (K ? (hi - lo) / K->slab_rows + 1 : 0));
     if (expect && P->n_partials < nblk) {
@@ -544,13 +555,13 @@ int bs_rows_apply(bs_plan* P, bs_sector* s, const double2* psi, double2* out, i6
         }
         dim3 fg(fgx, (unsigned)((r1 - r0 + 31) / 32));
         double2* part = expect ? P->d_partials.p + pdone : nullptr;
-        const double2* ot = T ? P->d_out_t.p : nullptr;
+        const double2* ot = need_t ? P->d_out_t.p : nullptr;
 #define BS_FINISH(E, TR) k_transpose_add_finish<E, TR><<<fg, 256, 0, st>>>(raw, ot, psi, out, Da, Db, r0, r1, ep, kc, part)
         if (expect) {
-            if (T) BS_FINISH(true, true);
+            if (need_t) BS_FINISH(true, true);
             else BS_FINISH(true, false);
         } else {
-            if (T) BS_FINISH(false, true);
+            if (need_t) BS_FINISH(false, true);
             else BS_FINISH(false, false);
         }
 #undef BS_FINISH

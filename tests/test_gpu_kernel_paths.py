@@ -76,6 +76,7 @@ for name, ref, raw, n, na, nb in cases + [('generic', None, (x, z, c), 6, 3, 2),
     assert want_kernel in desc or want_kernel == 'kres{', (want_kernel, desc)
     if name in ('q24', 'mol9') and want_kernel in ('rows_v2', 'kres{'):
         assert ('kres{' in desc) == (os.environ.get('BS_NO_KRES') is None), desc
+        assert ('k2{' in desc and 'k2_t{' in desc) == (os.environ.get('BS_NO_K2') is None), desc
     if name in ('hub10', 'hub10h', 'hubnnn') and want_kernel == 'rows_v2':
         assert ('+light' in desc) == (os.environ.get('BS_NO_LIGHT') is None), desc
     psi = si.random_state(osec.dim, 5)
@@ -103,7 +104,8 @@ print('PATH OK')
 
 @pytest.mark.parametrize("env,kernel", [
     ({}, "rows_v2"),
-    ({"BS_NO_LIGHT": "1", "BS_NO_KRES": "1"}, "rows_v2"),             # column-list pass instead of the K-resolved kernel
+    ({"BS_NO_LIGHT": "1", "BS_NO_KRES": "1", "BS_NO_K2": "1"}, "rows_v2"),   # column-list pass and row axpys only
+    ({"BS_K2_SLAB_MB": "1", "BS_K2_MIN": "1"}, "kres{"),              # several column slabs of the K2 scratch
     ({"BS_KRES_KC": "64", "BS_KRES_SLAB_MB": "2"}, "kres{"),          # more K chunks, several scratch slabs
     ({"BS_KRES_KC": "32", "BS_KRES_MIN": "1"}, "kres{"),
     ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0", "BS_LIGHT_SIGN": "1"}, "rows_v2"),   # light kernel: compacted list, one phase order, signed entries
