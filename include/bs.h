@@ -38,12 +38,15 @@
  *   - plan tables (row lists: 16 B per valid (alpha row, alpha mask) pair; column tables; 1.2 GB at config 5);
  *   - up to 3 state-vector-sized scratch buffers (transposed psi, transposed result, raw H psi) when beta-only
  *     groups run on the transposed problem (every molecular Hamiltonian): 3 x 16 x dim bytes (20 GB at config 5);
- *   - the scratch of the K-resolved alpha-beta kernel: n_orb x D_K x 16 bytes per alpha row of a slab, at most 4 GiB.
+ *   - the scratch of the K-resolved alpha-beta kernel: n_orb x D_K x 16 bytes per alpha row of a slab, at most 4 GiB,
+ *     plus its coupling matrices (<= 2.2 GB at config 5); the scratch of the K2-resolved same-spin kernels: 2 x 4 GiB.
  *
  * Environment (TEST HOOKS, not API; every one is read ONCE, when a plan is built, never on a launch path):
  *   BS_KERNEL=v1|v2inrow   force the v1 sector kernel / keep beta-only groups in-row
  *   BS_NO_LIGHT, BS_LIGHT_THREADS, BS_LIGHT_ORDER, BS_LIGHT_STREAM, BS_LIGHT_COMPACT, BS_LIGHT_SIGN   k_light variants
- *   BS_NO_KRES, BS_KRES_KC, BS_KRES_MIN, BS_KRES_SLAB_MB   K-resolved alpha-beta kernel off / chunk / threshold / slab
+ *   BS_NO_KRES, BS_KRES_KC, BS_KRES_MIN, BS_KRES_SLAB_MB, BS_KRES_MMA   K-resolved alpha-beta kernel off / chunk / threshold / slab / DFMA form
+ *   BS_NO_K2, BS_K2_MIN, BS_K2_SLAB_MB   K2-resolved same-spin double excitations off / threshold / slab
+ *   BS_ROT_IN_PLACE   rotation cells in place (L2) even when they fit shared memory; read per rotation call
  *   BS_ROW_WIN, BS_ROW_NO_SPLIT, BS_ROW_THREADS   k_rows source-row windows and block size
  *   BS_ROT_PER_LAUNCH   one launch per rotation generator (no closed-cell batching); read per rotation call
  */

@@ -81,10 +81,15 @@ k_aa(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i
 #pragma unroll
         for (int tt = 0; tt < RT; ++tt) acc[tt] = make_double2(0.0, 0.0);
         const double2* __restrict__ pc = psi + c;
-        for (int u = 0; u < P; u += 4) {
-            double2 a[4];   // four source rows in flight (rows beyond P read row 0 against a zero coupling row)
+        double2 a[4], an[4];   // four source rows being consumed, the next four in flight (rows beyond P read row 0
+                               // against a zero coupling row)
 #pragma unroll
-            for (int k = 0; k < 4; ++k) a[k] = __ldg(pc + (i64)srow[u + k] * L);
+        for (int k = 0; k < 4; ++k) a[k] = __ldg(pc + (i64)srow[k] * L);
+        for (int u = 0; u < P; u += 4) {
+            if (u + 4 < P) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) an[k] = __ldg(pc + (i64)srow[u + 4 + k] * L);
+            }
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const double2* __restrict__ g2 = reinterpret_cast<const double2*>(sC + (u + k) * RT);
@@ -97,6 +102,8 @@ k_aa(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i
                     acc[2 * t2 + 1].y += g.y * a[k].y;
                 }
             }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) a[k] = an[k];
         }
         double2* __restrict__ so = S2 + ((i64)f * P + t0) * W + (c - c0);
 #pragma unroll

@@ -21,27 +21,102 @@ constexpr int kMaxDenseStr = 160;     // strings of an absorbed x_b = 0 group (3
 constexpr int kMaxSegs = 48;          // staged column segments of a K chunk
 constexpr int kProducer = 32;         // threads of the producer warp (the last warp of the block)
 
-// register image of one header's tables in the producer warp, loaded one entry ahead of its use; the coupling-matrix
-// entries (lane, lane + 32, ...: at most NP of them) live in the registers the compute threads use as accumulators
-template <int NP>
-struct KresStage {
-    static constexpr int GQ = (NP * NP + 31) / 32, DQ = kMaxDenseStr / 32;
-    KresG d[DQ];   // strings of the absorbed x_b = 0 group (zero weight beyond the last)
-    u32 kr[2];     // string ranges (lo | hi << 8) of its keys lane and lane + 32
-};
+// shared-memory layout of one coupling matrix: row s holds G[s][0..NP), padded to a multiple of 8 columns (zero) and to a
+// row stride of 8 k + 4 doubles so that the four rows a half warp reads as an MMA fragment fall on different banks
+__host__ __device__ constexpr int kres_gs(int NP) { return (NP + 7) / 8 * 8 + 4; }
 
-template <int NP, int KCMAX>
+// Coupling matrices of rows [row_lo, ...): one block per target row, one warp per alpha mask (entry) of the row.
+// G[s][r] = V_{x_a,{r,s}}(t_a) from the header's tables (see the KresG codes), written in the padded shared-memory
+// layout of k_ab (row stride kres_gs) so that k_ab fetches a matrix with one bulk copy; every K chunk of the row reuses it.
+template <int NP>
+__global__ void __launch_bounds__(256)
+k_ab_g(const KresDev Kd, double* __restrict__ Gbuf, i64 row_lo) {
+    constexpr int GS = kres_gs(NP), GN = NP * GS, GQ = (NP * NP + 31) / 32, DQ = kMaxDenseStr / 32;
+    __shared__ double sVd_all[8][64], sStr_all[8][kMaxDenseStr];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double* sVd = sVd_all[w];
+    double* sStr = sStr_all[w];
+    const i64 row = row_lo + blockIdx.x;
+    const u32 ta = __ldg(Kd.a_str + row);
+    const i64 e0 = __ldg(Kd.row_off + row), e_base = __ldg(Kd.row_off + row_lo);
+    const int n_ent = (int)(__ldg(Kd.row_off + row + 1) - e0);
+    for (int i = w; i < n_ent; i += 8) {
+        const u32 kh = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i));
+        double* __restrict__ G = Gbuf + (e0 - e_base + i) * GN;
+        const KresG* __restrict__ gt = Kd.gtab + (size_t)kh * (NP * NP);
+        const KresG* __restrict__ ds = Kd.dstr + (size_t)kh * kMaxDenseStr;
+        const unsigned short* __restrict__ kr = Kd.dkr + (size_t)kh * 64;
+        const u32 kr0 = __ldg(kr + lane), kr1 = __ldg(kr + lane + 32);
+        // the absorbed x_b = 0 group: signed string weights, then one lane per key sums its strings in order;
+        // fixed-order butterfly for the total
+#pragma unroll
+        for (int q = 0; q < DQ; ++q) {
+            const KresG d = ds[lane + 32 * q];
+            sStr[lane + 32 * q] = flip(d.w, (u32)__popc(d.za & ta) & 1u);
+        }
+        __syncwarp();
+        // key 0 (beta Z mask 0) is the long one for a two-body Hamiltonian (n + 1 strings): the whole warp sums it;
+        // the other keys (one or two strings each) take one lane each
+        const u32 k0 = __shfl_sync(0xffffffffu, kr0, 0);
+        double v0 = 0.0;
+        for (u32 t = (k0 & 0xFFu) + lane; t < (k0 >> 8); t += 32) v0 += sStr[t];
+        for (int o = 16; o > 0; o >>= 1) v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+        double dsum = 0.0;
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+            const u32 krj = jj ? kr1 : kr0;
+            double v = 0.0;
+            if (jj == 0 && lane == 0) v = v0;
+            else
+                for (u32 t = krj & 0xFFu; t < (krj >> 8); ++t) v += sStr[t];
+            sVd[lane + 32 * jj] = v;
+            dsum += v;
+        }
+        for (int o = 16; o > 0; o >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, o);
+        __syncwarp();
+        auto V = [&](u32 key) {   // groups with several strings per key (not the JW case): from the plan tables
+            double f = 0.0;
+            const u32 s1 = __ldg(Kd.key_s0 + key + 1);
+            for (u32 s = __ldg(Kd.key_s0 + key); s < s1; ++s)
+                f += flip(__ldg(&Kd.s_w[s].x), (u32)__popc(__ldg(Kd.s_za + s) & ta) & 1u);
+            return f;
+        };
+#pragma unroll 4
+        for (int q = 0; q < GQ; ++q) {
+            const int p = lane + 32 * q;
+            if (p >= NP * NP) break;
+            const KresG g = gt[p];
+            const u32 type = g.code & kGType;
+            double v = 0.0;
+            if (type == kGSingle) v = flip(g.w, (u32)__popc(g.za & ta) & 1u);
+            else if (type == kGPair) {
+                v = V(g.code & kGKeyMask);
+                if (g.code & kGNeg) v = -v;
+            } else if (type == kGDiag) v = dsum * Kd.inv_nb;
+            else if (type == kGDiagKey) v = dsum * Kd.inv_nb - 2.0 * sVd[g.code & kGKeyMask];
+            G[(p / NP) * GS + p % NP] = v;
+        }
+        for (int q = lane; q < GN; q += 32)
+            if (q % GS >= NP) G[q] = 0.0;   // padding columns
+        __syncwarp();   // sStr / sVd are rewritten by the warp's next entry
+    }
+}
+
+// MMA: the contraction runs on the FP64 tensor instruction (mma.sync m8n8k4: same 64 FMA/clk/SM peak as DFMA, but one
+// G fragment load feeds 8 K rows and one instruction carries 256 FMA: a quarter of the shared-memory wavefronts and of
+// the issue slots of the DFMA form)
+template <int NP, int KCMAX, bool MMA>
 __global__ void __launch_bounds__(KCMAX + kProducer, 1)
-k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S, i64 row_lo) {
+k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict__ Gbuf, double2* __restrict__ S,
+     i64 row_lo) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double sVd[64], sStr[kMaxDenseStr];   // phase factors / signed string weights of the absorbed x_b = 0 group
-                                                     // (producer warp only)
     __shared__ uint2 sSeg[kMaxSegs];
     u64* bar = reinterpret_cast<u64*>(smem_raw);   // full[2] (producer + TMA -> compute warps), empty[2] (compute warps -> producer)
-    double* sG = reinterpret_cast<double*>(smem_raw + 32);                                   // [2][NP * NP]
-    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 32 + 2 * NP * NP * 8);             // [2][buf_elems]
+    constexpr int GS = kres_gs(NP), GN = NP * GS, NT = (NP + 7) / 8;
+    double* sG = reinterpret_cast<double*>(smem_raw + 32);                                   // [2][NP][GS]
+    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 32 + 2 * GN * 8);                  // [2][buf_elems]
     unsigned short* sgo =
-        reinterpret_cast<unsigned short*>(smem_raw + 32 + 2 * NP * NP * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
+        reinterpret_cast<unsigned short*>(smem_raw + 32 + 2 * GN * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
     const int tid = threadIdx.x, KC = (int)blockDim.x - kProducer;
     const bool producer = tid >= KC;
     const int lane = tid & 31;
@@ -62,46 +137,33 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
         for (int g = lane; g < nseg; g += 32) sSeg[g] = __ldg(Kd.segs + (size_t)chunk * Kd.max_segs + g);
     }
     if (tid == KC) {
-        mbar_init(bar, 2);       // full: the producer arrives twice (byte count of the copies; G written)
-        mbar_init(bar + 1, 2);
+        mbar_init(bar, 1);       // full: the producer's arrive.expect_tx; the bulk copies complete the byte count
+        mbar_init(bar + 1, 1);
         mbar_init(bar + 2, (u32)KC / 32);
         mbar_init(bar + 3, (u32)KC / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         sbuf[0] = make_double2(0.0, 0.0);             // position 0 of either buffer: the zero amplitude (s in K)
         sbuf[Kd.buf_elems] = make_double2(0.0, 0.0);
     }
-    double2 acc[NP];
+    constexpr int ACCN = MMA ? 16 * NT : NP;   // MMA: 4 K rows x NT column tiles x (re, im) fragments of two doubles
+    double2 acc[ACCN < NP ? NP : ACCN];
 #pragma unroll
-    for (int r = 0; r < NP; ++r) acc[r] = make_double2(0.0, 0.0);
+    for (int r = 0; r < (ACCN < NP ? NP : ACCN); ++r) acc[r] = make_double2(0.0, 0.0);
     const i64 e0 = __ldg(Kd.row_off + row);
     const int n_ent = (int)(__ldg(Kd.row_off + row + 1) - e0);
     const i64 Db = Kd.Db;
-    using Stage = KresStage<NP>;
+    const i64 e_base = __ldg(Kd.row_off + row_lo);
     u32 seg_bytes = 0;   // producer: bytes of one entry's bulk copies
 
     // ---- producer warp -----------------------------------------------------------------------------------------
-    // all table loads of entry i (addresses depend on the header id only) into registers; consumed one entry later
-    auto load = [&](Stage& st, int i) {
-        const u32 kh = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i));
-        const KresG* __restrict__ gt = Kd.gtab + (size_t)kh * (NP * NP);
-#pragma unroll
-        for (int q = 0; q < Stage::GQ; ++q) {
-            const int p = lane + 32 * q;
-            if (p < NP * NP) acc[q] = *reinterpret_cast<const double2*>(gt + p);   // {w, (za, code)} as 16 raw bytes
-        }
-        const KresG* __restrict__ ds = Kd.dstr + (size_t)kh * kMaxDenseStr;
-#pragma unroll
-        for (int q = 0; q < Stage::DQ; ++q) st.d[q] = ds[lane + 32 * q];
-        const unsigned short* __restrict__ kr = Kd.dkr + (size_t)kh * 64;
-        st.kr[0] = __ldg(kr + lane);
-        st.kr[1] = __ldg(kr + lane + 32);
-    };
     // TMA bulk copies of the chunk's column segments of entry i's source row into buffer i & 1 (lane 0)
     auto stage_row = [&](int i) {
         const u32 src_row = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i) + 1);
         const double2* __restrict__ src = psi + (i64)src_row * Db;
         unsigned char* dst = reinterpret_cast<unsigned char*>(sbuf + (size_t)(i & 1) * Kd.buf_elems + 1);
-        mbar_expect_tx(bar + (i & 1), seg_bytes);
+        mbar_expect_tx(bar + (i & 1), seg_bytes + (u32)(GN * 8));
+        // the entry's coupling matrix, made by k_ab_g for all K chunks of the row
+        tma_bulk_g2s(sG + (i & 1) * GN, Gbuf + (e0 - e_base + i) * GN, (u32)(GN * 8), bar + (i & 1));
         for (int g = 0; g < nseg; ++g) {
             const uint2 sg = sSeg[g];
             const unsigned char* sp = reinterpret_cast<const unsigned char*>(src + sg.x);
@@ -110,83 +172,86 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
             dst += bytes;
         }
     };
-    // coupling matrix G[i & 1] of entry i from its register image
-    auto make_g = [&](const Stage& st, int i) {
-        double* G = sG + (i & 1) * (NP * NP);
-        // the absorbed x_b = 0 group: signed string weights, then one lane per key sums its strings in order;
-        // fixed-order butterfly for the total
-#pragma unroll
-        for (int q = 0; q < Stage::DQ; ++q) sStr[lane + 32 * q] = flip(st.d[q].w, (u32)__popc(st.d[q].za & ta) & 1u);
-        __syncwarp();
-        // key 0 (beta Z mask 0) is the long one for a two-body Hamiltonian (n + 1 strings): the whole warp sums it;
-        // the other keys (one or two strings each) take one lane each
-        const u32 k0 = __shfl_sync(0xffffffffu, st.kr[0], 0);
-        double v0 = 0.0;
-        for (u32 t = (k0 & 0xFFu) + lane; t < (k0 >> 8); t += 32) v0 += sStr[t];
-        for (int o = 16; o > 0; o >>= 1) v0 += __shfl_xor_sync(0xffffffffu, v0, o);
-        double dsum = 0.0;
-#pragma unroll
-        for (int jj = 0; jj < 2; ++jj) {
-            double v = 0.0;
-            if (jj == 0 && lane == 0) v = v0;
-            else
-                for (u32 t = st.kr[jj] & 0xFFu; t < (st.kr[jj] >> 8); ++t) v += sStr[t];
-            sVd[lane + 32 * jj] = v;
-            dsum += v;
-        }
-        for (int o = 16; o > 0; o >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, o);
-        __syncwarp();
-        auto V = [&](u32 key) {   // groups with several strings per key (not the JW case): from the plan tables
-            double f = 0.0;
-            const u32 s1 = __ldg(Kd.key_s0 + key + 1);
-            for (u32 s = __ldg(Kd.key_s0 + key); s < s1; ++s)
-                f += flip(__ldg(&Kd.s_w[s].x), (u32)__popc(__ldg(Kd.s_za + s) & ta) & 1u);
-            return f;
-        };
-#pragma unroll
-        for (int q = 0; q < Stage::GQ; ++q) {
-            const int p = lane + 32 * q;
-            if (p >= NP * NP) break;
-            KresG g;
-            g.w = acc[q].x;
-            g.za = (u32)__double2loint(acc[q].y);
-            g.code = (u32)__double2hiint(acc[q].y);
-            const u32 type = g.code & kGType;
-            double v = 0.0;
-            if (type == kGSingle) v = flip(g.w, (u32)__popc(g.za & ta) & 1u);
-            else if (type == kGPair) {
-                v = V(g.code & kGKeyMask);
-                if (g.code & kGNeg) v = -v;
-            } else if (type == kGDiag) v = dsum * Kd.inv_nb;
-            else if (type == kGDiagKey) v = dsum * Kd.inv_nb - 2.0 * sVd[g.code & kGKeyMask];
-            G[p] = v;
-        }
-        __syncwarp();   // sStr / sVd are rewritten by the next entry; G is complete
-        // the producer's second arrival on full[i & 1] (release: G is visible to whoever observes the phase)
-        if (lane == 0) mbar_arrive(bar + (i & 1));
-    };
-    Stage st;
     __syncthreads();
     if (producer) {
         // No block barrier in the entry loop: the producer refills buffer b as soon as every compute warp has released
         // it (empty[b]); a compute warp starts entry i as soon as full[i & 1] completes, whatever the other warps do.
-        for (int g = 0; g < nseg; ++g) seg_bytes += sSeg[g].y * 16u;
-        if (n_ent > 0) load(st, 0);
-        for (int i = 0; i < n_ent; ++i) {
-            if (i >= 2) mbar_wait(bar + 2 + (i & 1), (u32)((i >> 1) - 1) & 1u);
-            if (lane == 0) stage_row(i);
-            make_g(st, i);
-            if (i + 1 < n_ent) load(st, i + 1);   // lands while this warp waits for the next free buffer
+        if (lane == 0) {
+            for (int g = 0; g < nseg; ++g) seg_bytes += sSeg[g].y * 16u;
+            for (int i = 0; i < n_ent; ++i) {
+                if (i >= 2) mbar_wait(bar + 2 + (i & 1), (u32)((i >> 1) - 1) & 1u);
+                stage_row(i);
+            }
         }
         return;
     }
-    // orbitals with a source K + {s} for some K of this warp, walked in ascending order (warp-uniform); the gather of
-    // the next orbital is issued before the DFMA block of the current one
+    // orbitals with a source K + {s} for some K of this warp (warp-uniform set)
     const u32 act_all = ~in_k & (Kd.n >= 32 ? 0xFFFFFFFFu : ((1u << Kd.n) - 1u));
+    if (MMA) {
+        // Warp tile: 32 K rows (this warp's K) x NP columns; fragment coordinates g = lane / 4, tq = lane % 4.
+        // A[K][s] = sigma_s(K) psi[u_a, K + {s}] (re and im as separate row tiles), B[s][r] = G[s][r], four active
+        // orbitals per step.  Row tile i holds K = 32 w + 8 i + g.
+        const int g = lane >> 2, tq = lane & 3, kw = (tid & ~31) + g;
+        u32 sigk[4];
+#pragma unroll
+        for (int i2 = 0; i2 < 4; ++i2) sigk[i2] = __shfl_sync(0xffffffffu, sig, 8 * i2 + g);
+        const int n_act = __popc(act_all);
+        for (int i = 0; i < n_ent; ++i) {
+            mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
+            const double* __restrict__ G = sG + (i & 1) * GN;
+            const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
+            for (int ks = 0; ks < n_act; ks += 4) {
+                const u32 s = __fns(act_all, 0, ks + tq + 1);   // this lane's orbital of the step (0xFFFFFFFF: none left)
+                const bool valid = s < 32u;
+                const u32 sc = valid ? s : 0u;
+                double are[4], aim[4], bf[NT];
+#pragma unroll
+                for (int i2 = 0; i2 < 4; ++i2) {
+                    const double2 b = buf[valid ? sgo[sc * KC + kw + 8 * i2] : 0];
+                    const u32 sg = (sigk[i2] >> sc) & 1u;
+                    are[i2] = flip(b.x, sg);
+                    aim[i2] = flip(b.y, sg);
+                }
+#pragma unroll
+                for (int j = 0; j < NT; ++j) bf[j] = valid ? G[sc * GS + 8 * j + g] : 0.0;
+#pragma unroll
+                for (int i2 = 0; i2 < 4; ++i2)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) {
+                        double2& cr = acc[(i2 * NT + j) * 2];
+                        double2& ci = acc[(i2 * NT + j) * 2 + 1];
+                        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                     : "+d"(cr.x), "+d"(cr.y) : "d"(are[i2]), "d"(bf[j]));
+                        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                     : "+d"(ci.x), "+d"(ci.y) : "d"(aim[i2]), "d"(bf[j]));
+                    }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar + 2 + (i & 1));   // this warp is done with buffer i & 1
+        }
+        // C fragment: row g of tile i2 (K = kw + 8 i2), columns 8 j + 2 tq + {0, 1}
+#pragma unroll
+        for (int i2 = 0; i2 < 4; ++i2)
+#pragma unroll
+            for (int j = 0; j < NT; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int r = 8 * j + 2 * tq + e;
+                    if (r < Kd.n) {
+                        const u32 sg = (sigk[i2] >> r) & 1u;
+                        const double2 cr = acc[(i2 * NT + j) * 2], ci = acc[(i2 * NT + j) * 2 + 1];
+                        S[((i64)blockIdx.x * Kd.n + r) * Kd.DKp + (i64)chunk * KC + kw + 8 * i2] =
+                            make_double2(flip(e ? cr.y : cr.x, sg), flip(e ? ci.y : ci.x, sg));
+                    }
+                }
+        return;
+    }
+    // DFMA form: orbitals walked in ascending order; the gather of the next orbital is issued before the DFMA block of
+    // the current one
     const unsigned short* __restrict__ my_go = sgo + tid;
     for (int i = 0; i < n_ent; ++i) {
         mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
-        const double* __restrict__ G = sG + (i & 1) * (NP * NP);
+        const double* __restrict__ G = sG + (i & 1) * GN;
         const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
         u32 act = act_all;
         int s = __ffs((int)act) - 1;
@@ -200,10 +265,10 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, double2* __restrict__ S,
             const u32 sg = (sig >> s) & 1u;
             b.x = flip(b.x, sg);
             b.y = flip(b.y, sg);
-            const double2* __restrict__ g2 = reinterpret_cast<const double2*>(G + s * NP);
+            const double2* __restrict__ g2 = reinterpret_cast<const double2*>(G + s * GS);
 #pragma unroll
             for (int r2 = 0; r2 < NP / 2; ++r2) {
-                const double2 g = g2[r2];   // warp-uniform address: one broadcast wavefront for two columns of G
+                const double2 g = g2[r2];   // warp-uniform address: two wavefronts for two columns of G
                 acc[2 * r2].x += g.x * b.x;
                 acc[2 * r2].y += g.x * b.y;
                 acc[2 * r2 + 1].x += g.y * b.x;
@@ -231,10 +296,11 @@ constexpr int kres_kcmax(int NP) { return NP <= 16 ? 480 : 224; }
 
 template <int NP>
 cudaError_t kab_launch(const bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st, bool set_attr) {
-    auto k = k_ab<NP, kres_kcmax(NP)>;
+    auto k = K->mma ? k_ab<NP, kres_kcmax(NP), true> : k_ab<NP, kres_kcmax(NP), false>;
     if (set_attr) return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K->smem);
     dim3 grid((unsigned)(hi - lo), (unsigned)K->n_chunks);
-    k<<<grid, K->KC + kProducer, K->smem, st>>>(K->dev, psi, K->d_S.p, lo);
+    k_ab_g<NP><<<(unsigned)(hi - lo), 256, 0, st>>>(K->dev, K->d_G.p, lo);
+    k<<<grid, K->KC + kProducer, K->smem, st>>>(K->dev, psi, K->d_G.p, K->d_S.p, lo);
     return cudaGetLastError();
 }
 
@@ -426,7 +492,7 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
                     goff[((size_t)c * NP + s) * KC + (k - (i64)c * KC)] = (unsigned short)(base[g] + (col - sg[g].x));
                 }
         }
-        const size_t smem = 32 + 2 * (size_t)NP * NP * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
+        const size_t smem = 32 + 2 * (size_t)NP * kres_gs(NP) * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
         if (smem <= smem_max && buf_elems <= 65535) {
             K->smem = smem;
             segs.assign((size_t)n_chunks * max_segs, make_uint2(0u, 0u));
@@ -439,6 +505,7 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
         }
     }
     K->KC = KC;
+    K->mma = getenv("BS_KRES_MMA") ? atoi(getenv("BS_KRES_MMA")) != 0 : true;   // test hook: 0 = DFMA form
     K->n_chunks = n_chunks;
     K->max_segs = max_segs;
     K->buf_elems = buf_elems;
@@ -469,7 +536,16 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
     i64 budget = i64(4) << 30;
     if (const char* e = getenv("BS_KRES_SLAB_MB")) budget = std::max<i64>(1, atoll(e)) << 20;   // test hook
     K->slab_rows = std::max<i64>(1, std::min<i64>(S->Da, budget / per_row));
-    cudaError_t ce = K->d_S.alloc((size_t)(K->slab_rows * n * K->DKp));
+    // coupling matrices of one slab (k_ab_g): the most entries any slab of slab_rows rows holds
+    std::vector<i64> h_off(S->Da + 1);
+    cudaError_t ce = cudaMemcpyAsync(h_off.data(), R->d_row_off.p, (S->Da + 1) * 8, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    i64 max_ent = 1;
+    for (i64 r0 = 0; r0 < S->Da; r0 += K->slab_rows)
+        max_ent = std::max(max_ent, h_off[std::min<i64>(S->Da, r0 + K->slab_rows)] - h_off[r0]);
+    K->g_bytes = (size_t)max_ent * NP * kres_gs(NP) * 8;
+    if (ce == cudaSuccess) ce = K->d_G.alloc((size_t)max_ent * NP * kres_gs(NP));
+    if (ce == cudaSuccess) ce = K->d_S.alloc((size_t)(K->slab_rows * n * K->DKp));
     if (ce == cudaSuccess) ce = K->d_gtab.upload(gtab, st);
     if (ce == cudaSuccess) ce = K->d_dstr.upload(dstr, st);
     if (ce == cudaSuccess) ce = K->d_dkr.upload(dkr, st);
@@ -517,6 +593,6 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
 // rows [lo, hi) (at most slab_rows) -> scratch S[row - lo][r][K]
 int bs_kres_apply(bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st) {
     BS_CUDA(kab_dispatch(K, psi, lo, hi, st, false));
-    BS_COUNT_LAUNCH(1);
+    BS_COUNT_LAUNCH(2);
     return BS_OK;
 }

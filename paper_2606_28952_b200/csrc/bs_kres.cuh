@@ -10,7 +10,8 @@
 // so that for a fixed source row u_a = t_a ^ x_a
 //   out[t_a, K + {r}] += sigma_r(K) * sum_s G[s][r] * ( sigma_s(K) psi[u_a, K + {s}] ),
 //   G[s][r] = V_{x_a,{r,s}}(t_a) (times the constant sign of zb_g's own bits on r, s), G[r][r] from the x_b = 0 group.
-// A producer warp evaluates G for the next alpha mask and issues the TMA copies while the other warps compute.
+// A small kernel (k_ab_g) evaluates G for every (row, alpha mask) of a slab once -- all K chunks of the row reuse it --
+// and a producer warp of k_ab fetches it with the column segments by TMA while the other warps compute.
 // One thread owns one K and keeps all n accumulators (one per r) in registers over ALL alpha masks of its row:
 // every gathered amplitude psi[u_a, K + {s}] feeds n - N_beta + 1 targets (the column-list pass of k_rows gathers it
 // once per target), G comes from shared memory by warp-uniform (broadcast) loads, and the inner loop is plain DFMA:
@@ -62,6 +63,7 @@ struct bs_kres {
     int n = 0, NP = 0, Nb = 0, KC = 0, n_chunks = 0, max_segs = 0, buf_elems = 0;
     i64 DK = 0, DKp = 0, slab_rows = 0;
     size_t smem = 0;
+    bool mma = true;             // contraction on the FP64 tensor instruction (else DFMA)
     double staged_rows = 0;      // staged columns per alpha mask, in units of one source row (bs_plan_describe)
     DevBuf<KresG> d_gtab;
     DevBuf<u32> d_sigma, d_comb;
@@ -70,6 +72,8 @@ struct bs_kres {
     DevBuf<uint2> d_segs;
     DevBuf<int> d_segcnt;
     DevBuf<unsigned short> d_goff;
+    DevBuf<double> d_G;          // coupling matrices of one slab, one per (row, alpha mask) (k_ab_g)
+    size_t g_bytes = 0;
     DevBuf<double2> d_S;         // scratch for slab_rows rows (allocated at plan build, size in bs_plan_describe)
     KresDev dev{};
     ~bs_kres();
