@@ -48,7 +48,8 @@ __global__ void __launch_bounds__(kAaThreads)
 k_aa(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i64 L, i64 c0, i64 W, i64 row_lo,
      i64 row_hi) {
     extern __shared__ __align__(16) unsigned char smem_k2[];
-    const int P = K.P, f = blockIdx.x, t0 = blockIdx.y * RT, nt = min(RT, P - t0), tid = threadIdx.x;
+    // the tiles of one family are neighbours in launch order: they stream the same source rows, which L2 then serves
+    const int P = K.P, f = blockIdx.y, t0 = blockIdx.x * RT, nt = min(RT, P - t0), tid = threadIdx.x;
     double* sC = reinterpret_cast<double*>(smem_k2);                       // [P + 4][RT] coupling tile, source-major
     u32* srow = reinterpret_cast<u32*>(smem_k2 + (size_t)(P + 4) * RT * 8);  // [P + 4] row of every source member
     const u32* __restrict__ mrow = K.mrow + (size_t)f * P;
@@ -137,7 +138,7 @@ template <int RT>
 cudaError_t kaa_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi, cudaStream_t st,
                        bool set_attr) {
     if (set_attr) return cudaFuncSetAttribute(k_aa<RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K->smem);
-    dim3 grid((unsigned)K->F, (unsigned)K->n_tiles);
+    dim3 grid((unsigned)K->n_tiles, (unsigned)K->F);
     k_aa<RT><<<grid, kAaThreads, K->smem, st>>>(K->dev, psi, K->d_S2.p, L, c0, W, row_lo, row_hi);
     return cudaGetLastError();
 }
@@ -239,11 +240,13 @@ int bs_k2_build(std::vector<HostGroup>& groups, const std::vector<u64>& row_stri
     K->NP2 = NP2;
     K->rows = rows;
     K->n_groups = n_q;
-    const int tiles0 = (P + 27) / 28;
-    K->rt = std::min(28, std::max(4, (((P + tiles0 - 1) / tiles0) + 3) / 4 * 4));
+    // 12 targets per tile: 2 x 12 DFMA per 16-byte load still hides the load behind arithmetic, and at ~100 registers two
+    // blocks (16 warps) fit an SM; 28-target tiles (1 block, 8 warps) were 3 - 6 % slower on configs 2, 4 and 5
+    K->rt = std::min(12, (P + 3) / 4 * 4);
+    if (const char* e = getenv("BS_K2_RT")) K->rt = std::min(28, std::max(4, atoi(e) / 4 * 4));   // test hook: tile height
     K->n_tiles = (P + K->rt - 1) / K->rt;
     K->smem = (size_t)(P + 4) * K->rt * 8 + (size_t)(P + 4) * 4;
-    if (K->smem > 200 * 1024 || (i64)F * P >= (i64(1) << 31)) {
+    if (K->smem > 200 * 1024 || (i64)F * P >= (i64(1) << 31) || F > 65535) {
         delete K;
         return BS_OK;
     }

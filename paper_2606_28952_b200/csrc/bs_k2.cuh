@@ -7,9 +7,9 @@
 //   out[K2 + pair_t, c] += sum_{pair_u disjoint from pair_t} F_g(K2 + pair_t) psi[K2 + pair_u, c],   x_g = pair_t | pair_u,
 // F_g(t) = sum_k w_k (-1)^{popc(z_k & t)} the group's phase sum (Eq. 27).  The row kernel reads one source amplitude
 // from L2 per non-zero (28 x 28 = 784 source rows per target row at configs[3], 1,656 at configs[4]: it runs at the
-// L2 -> SM bandwidth).  Here a thread block owns (family, tile of <= 28 target rows): one thread per column keeps the
+// L2 -> SM bandwidth).  Here a thread block owns (family, tile of 12 target rows): one thread per column keeps the
 // tile's accumulators in registers and every source amplitude it loads (coalesced, one row after the other) feeds all
-// targets of the tile, with the coupling tile broadcast from shared memory -- 2 x 28 DFMA per 16-byte load.  A target
+// targets of the tile, with the coupling tile broadcast from shared memory -- 2 x 12 DFMA per 16-byte load.  A target
 // row belongs to C(N, 2) families; the blocks write their tiles to a scratch S2[family][member][column] and a second
 // kernel adds the C(N, 2) contributions of every target in a fixed order (deterministic, no atomics), column slab by
 // column slab so that the scratch stays bounded.
