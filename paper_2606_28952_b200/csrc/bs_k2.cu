@@ -137,7 +137,8 @@ k_aa_acc(const u32* __restrict__ tf, int NP2, const double2* __restrict__ S2, do
 template <int RT>
 cudaError_t kaa_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi, cudaStream_t st,
                        bool set_attr) {
-    if (set_attr) return cudaFuncSetAttribute(k_aa<RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K->smem);
+    if (set_attr) return cudaFuncSetAttribute(k_aa<RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);   // the ceiling is per kernel,
+                                                                  // shared by all plans: never lower it to one plan's size
     dim3 grid((unsigned)K->n_tiles, (unsigned)K->F);
     k_aa<RT><<<grid, kAaThreads, K->smem, st>>>(K->dev, psi, K->d_S2.p, L, c0, W, row_lo, row_hi);
     return cudaGetLastError();

@@ -105,8 +105,16 @@ k_ab_g(const KresDev Kd, double* __restrict__ Gbuf, i64 row_lo) {
 // MMA: the contraction runs on the FP64 tensor instruction (mma.sync m8n8k4: same 64 FMA/clk/SM peak as DFMA, but one
 // G fragment load feeds 8 K rows and one instruction carries 256 FMA: a quarter of the shared-memory wavefronts and of
 // the issue slots of the DFMA form)
+// row tiles (8 K each) per warp of the MMA form: 4 up to 16 orbitals; 2 above, where 4 would need > 200 registers and leave
+// 7 compute warps per SM (2 tiles: 14 warps at <= 128 registers)
+__host__ __device__ constexpr int kres_rtw(int NP) { return NP <= 16 ? 4 : 2; }
+// threads per block: DFMA form one thread per K; MMA form one warp per 8 * rtw K; + the producer warp
+__host__ __device__ constexpr int kres_threads(int NP, int KC, bool mma) {
+    return (mma ? KC / (8 * kres_rtw(NP)) * 32 : KC) + 32;
+}
+
 template <int NP, int KCMAX, bool MMA>
-__global__ void __launch_bounds__(KCMAX + kProducer, 1)
+__global__ void __launch_bounds__(kres_threads(NP, KCMAX, MMA), 1)
 k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict__ Gbuf, double2* __restrict__ S,
      i64 row_lo) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -117,8 +125,9 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
     double2* sbuf = reinterpret_cast<double2*>(smem_raw + 32 + 2 * GN * 8);                  // [2][buf_elems]
     unsigned short* sgo =
         reinterpret_cast<unsigned short*>(smem_raw + 32 + 2 * GN * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
-    const int tid = threadIdx.x, KC = (int)blockDim.x - kProducer;
-    const bool producer = tid >= KC;
+    constexpr int RTW = kres_rtw(NP);
+    const int tid = threadIdx.x, KC = Kd.KC, n_cmp = (int)blockDim.x - kProducer;   // K per chunk, compute threads
+    const bool producer = tid >= n_cmp;
     const int lane = tid & 31;
     const i64 row = row_lo + blockIdx.x;
     const int chunk = blockIdx.y;
@@ -126,26 +135,21 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
     const int nseg = __ldg(Kd.seg_cnt + chunk);
     u32 sig = 0, in_k = 0;   // in_k: orbitals that every K of this warp holds (no source, no target there: skipped)
     if (!producer) {
-        sig = __ldg(Kd.sigma + (size_t)chunk * KC + tid);
-        for (int s = 0; s < NP; ++s) {
-            const unsigned short o = __ldg(Kd.goff + ((size_t)chunk * NP + s) * KC + tid);
-            sgo[s * KC + tid] = o;
-            in_k |= (o == 0 ? 1u : 0u) << s;
-        }
-        in_k = __reduce_and_sync(0xffffffffu, in_k);
+        if (!MMA) sig = __ldg(Kd.sigma + (size_t)chunk * KC + tid);
+        for (int idx = tid; idx < NP * KC; idx += n_cmp) sgo[idx] = __ldg(Kd.goff + (size_t)chunk * NP * KC + idx);
     } else {
         for (int g = lane; g < nseg; g += 32) sSeg[g] = __ldg(Kd.segs + (size_t)chunk * Kd.max_segs + g);
     }
-    if (tid == KC) {
+    if (tid == n_cmp) {
         mbar_init(bar, 1);       // full: the producer's arrive.expect_tx; the bulk copies complete the byte count
         mbar_init(bar + 1, 1);
-        mbar_init(bar + 2, (u32)KC / 32);
-        mbar_init(bar + 3, (u32)KC / 32);
+        mbar_init(bar + 2, (u32)n_cmp / 32);
+        mbar_init(bar + 3, (u32)n_cmp / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         sbuf[0] = make_double2(0.0, 0.0);             // position 0 of either buffer: the zero amplitude (s in K)
         sbuf[Kd.buf_elems] = make_double2(0.0, 0.0);
     }
-    constexpr int ACCN = MMA ? 16 * NT : NP;   // MMA: 4 K rows x NT column tiles x (re, im) fragments of two doubles
+    constexpr int ACCN = MMA ? 4 * RTW * NT : NP;   // MMA: RTW row tiles x NT column tiles x (re, im) fragments of two doubles
     double2 acc[ACCN < NP ? NP : ACCN];
 #pragma unroll
     for (int r = 0; r < (ACCN < NP ? NP : ACCN); ++r) acc[r] = make_double2(0.0, 0.0);
@@ -185,16 +189,28 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
         }
         return;
     }
-    // orbitals with a source K + {s} for some K of this warp (warp-uniform set)
+    // orbitals that every K of this warp holds have no source and no target there: skipped warp-uniformly
+    if (MMA) {
+        const int g0 = lane >> 2, tq0 = lane & 3, kw0 = (tid >> 5) * (8 * RTW) + g0;
+        in_k = 0xFFFFFFFFu;
+        for (int s = tq0; s < NP; s += 4) {
+            bool all = true;
+            for (int i2 = 0; i2 < RTW; ++i2) all &= sgo[s * KC + kw0 + 8 * i2] == 0;
+            if (!all) in_k &= ~(1u << s);
+        }
+    } else {
+        for (int s = 0; s < NP; ++s) in_k |= (sgo[s * KC + tid] == 0 ? 1u : 0u) << s;
+    }
+    in_k = __reduce_and_sync(0xffffffffu, in_k);
     const u32 act_all = ~in_k & (Kd.n >= 32 ? 0xFFFFFFFFu : ((1u << Kd.n) - 1u));
     if (MMA) {
         // Warp tile: 32 K rows (this warp's K) x NP columns; fragment coordinates g = lane / 4, tq = lane % 4.
         // A[K][s] = sigma_s(K) psi[u_a, K + {s}] (re and im as separate row tiles), B[s][r] = G[s][r], four active
-        // orbitals per step.  Row tile i holds K = 32 w + 8 i + g.
-        const int g = lane >> 2, tq = lane & 3, kw = (tid & ~31) + g;
-        u32 sigk[4];
+        // orbitals per step.  Row tile i of warp w holds K = 8 RTW w + 8 i + g.
+        const int g = lane >> 2, tq = lane & 3, kw = (tid >> 5) * (8 * RTW) + g;
+        u32 sigk[RTW];
 #pragma unroll
-        for (int i2 = 0; i2 < 4; ++i2) sigk[i2] = __shfl_sync(0xffffffffu, sig, 8 * i2 + g);
+        for (int i2 = 0; i2 < RTW; ++i2) sigk[i2] = __ldg(Kd.sigma + (size_t)chunk * KC + kw + 8 * i2);
         const int n_act = __popc(act_all);
         for (int i = 0; i < n_ent; ++i) {
             mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
@@ -204,9 +220,9 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
                 const u32 s = __fns(act_all, 0, ks + tq + 1);   // this lane's orbital of the step (0xFFFFFFFF: none left)
                 const bool valid = s < 32u;
                 const u32 sc = valid ? s : 0u;
-                double are[4], aim[4], bf[NT];
+                double are[RTW], aim[RTW], bf[NT];
 #pragma unroll
-                for (int i2 = 0; i2 < 4; ++i2) {
+                for (int i2 = 0; i2 < RTW; ++i2) {
                     const double2 b = buf[valid ? sgo[sc * KC + kw + 8 * i2] : 0];
                     const u32 sg = (sigk[i2] >> sc) & 1u;
                     are[i2] = flip(b.x, sg);
@@ -215,7 +231,7 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
 #pragma unroll
                 for (int j = 0; j < NT; ++j) bf[j] = valid ? G[sc * GS + 8 * j + g] : 0.0;
 #pragma unroll
-                for (int i2 = 0; i2 < 4; ++i2)
+                for (int i2 = 0; i2 < RTW; ++i2)
 #pragma unroll
                     for (int j = 0; j < NT; ++j) {
                         double2& cr = acc[(i2 * NT + j) * 2];
@@ -231,7 +247,7 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
         }
         // C fragment: row g of tile i2 (K = kw + 8 i2), columns 8 j + 2 tq + {0, 1}
 #pragma unroll
-        for (int i2 = 0; i2 < 4; ++i2)
+        for (int i2 = 0; i2 < RTW; ++i2)
 #pragma unroll
             for (int j = 0; j < NT; ++j)
 #pragma unroll
@@ -297,10 +313,11 @@ constexpr int kres_kcmax(int NP) { return NP <= 16 ? 480 : 224; }
 template <int NP>
 cudaError_t kab_launch(const bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st, bool set_attr) {
     auto k = K->mma ? k_ab<NP, kres_kcmax(NP), true> : k_ab<NP, kres_kcmax(NP), false>;
-    if (set_attr) return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K->smem);
+    // the ceiling is per kernel and shared by all plans: the opt-in maximum minus the kernel's static shared memory
+    if (set_attr) return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
     dim3 grid((unsigned)(hi - lo), (unsigned)K->n_chunks);
     k_ab_g<NP><<<(unsigned)(hi - lo), 256, 0, st>>>(K->dev, K->d_G.p, lo);
-    k<<<grid, K->KC + kProducer, K->smem, st>>>(K->dev, psi, K->d_G.p, K->d_S.p, lo);
+    k<<<grid, kres_threads(NP, K->KC, K->mma), K->smem, st>>>(K->dev, psi, K->d_G.p, K->d_S.p, lo);
     return cudaGetLastError();
 }
 

@@ -308,10 +308,10 @@ static int env_int(const char* name, int dflt) {
 template <int MODE, bool SIGN>
 static cudaError_t light_set_smem(int maxt, size_t smem) {
     switch (maxt) {
-        case 512: return cudaFuncSetAttribute(k_light<MODE, 512, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        case 768: return cudaFuncSetAttribute(k_light<MODE, 768, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        case 896: return cudaFuncSetAttribute(k_light<MODE, 896, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        default: return cudaFuncSetAttribute(k_light<MODE, 1024, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        case 512: return cudaFuncSetAttribute(k_light<MODE, 512, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+        case 768: return cudaFuncSetAttribute(k_light<MODE, 768, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+        case 896: return cudaFuncSetAttribute(k_light<MODE, 896, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
+        default: return cudaFuncSetAttribute(k_light<MODE, 1024, SIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
     }
 }
 
