@@ -159,6 +159,19 @@ int bs_expect(bs_op_t op, bs_sector_t s, const void* psi, double result_reim[2],
 /* <a|b> = sum conj(a_i) b_i over dim amplitudes, same deterministic reduction.  Synchronises. */
 int bs_vdot(bs_sector_t s, const void* a, const void* b, double result_reim[2], void* cuda_stream);
 
+/* ---- no-allocation variant of bs_vdot, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops):
+ * result_dev [device] double[2] <- sum_i conj(a_i) b_i over n amplitudes; a, b [device] complex128[n], 16-byte aligned.
+ * The per-block partial sums live in a 128 KiB file-scope __device__ array (every GPU that loads the library holds it
+ * until exit) instead of malloc'ed scratch: 8192 partials of 65,536 amplitudes each, so n <= bs_noalloc_max_dim() =
+ * 536,870,912; longer vectors return BS_ERR_ARG.  The call allocates nothing, copies nothing to the host and does not
+ * synchronise (two launches on cuda_stream).  bs_noalloc_setup takes the array's device address for the CURRENT device,
+ * once per device; bs_vdot_noalloc calls it on first use, but under graph capture call it beforehand.  Every call on a
+ * device shares the array: calls that overlap on the GPU (other streams, concurrent graph replays) race -- one stream
+ * at a time.  Stale contents are harmless: a call reads only the partials it has just written.  Deterministic. */
+int bs_noalloc_setup(void);
+int64_t bs_noalloc_max_dim(void);
+int bs_vdot_noalloc(const void* a, const void* b, int64_t n, void* result_dev, void* cuda_stream);
+
 /* ---- a6: psi <- exp(theta_j A_j) psi for j = 0..n_rot-1 in order, A_j = group j of a
  * BS_MODE_SEQUENCE operator: anti-Hermitian (every c_k purely imaginary), one x, mutually
  * commuting strings (Eq. 39).  x = 0 (diagonal generator, e.g. exp(-i w Z_j Z_{j+1}) of

@@ -27,7 +27,7 @@ SYMBOLS = [
     "bs_apply", "bs_apply_rows", "bs_apply_axpby", "bs_expect", "bs_vdot",
     "bs_apply_pauli_rotations", "bs_taylor_step", "bs_plan_describe", "bs_plan_info", "bs_plan_groups",
     "bs_symsector_build", "bs_symsector_info", "bs_symsector_destroy", "bs_sym_scatter", "bs_sym_gather", "bs_sym_apply",
-    "bs_sym_expect", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
+    "bs_sym_expect", "bs_noalloc_setup", "bs_noalloc_max_dim", "bs_vdot_noalloc", "bs_jw_molecular", "bs_jw_hubbard", "bs_launch_count", "bs_last_error", "bs_version",
 ]
 
 
@@ -70,6 +70,9 @@ def _load():
     L.bs_sym_gather.argtypes = [vp, vp, vp, vp]
     L.bs_sym_apply.argtypes = [vp, vp, vp, vp, vp]
     L.bs_sym_expect.argtypes = [vp, vp, vp, C.POINTER(dbl), vp]
+    L.bs_noalloc_setup.argtypes = []
+    L.bs_noalloc_max_dim.restype = i64
+    L.bs_vdot_noalloc.argtypes = [vp, vp, i64, vp, vp]
     L.bs_plan_info.argtypes = [vp, vp, C.POINTER(i64), vp]
     L.bs_plan_groups.argtypes = [vp, vp, vp, vp, i64, C.POINTER(i64), vp]
     L.bs_launch_count.restype = i64
@@ -243,6 +246,22 @@ def bs_vdot(sector: Sector, a, b, stream=None) -> complex:
     _check(_lib.bs_vdot(sector._h, _dev_ptr(a, sector.dim, "a"), _dev_ptr(b, sector.dim, "b"), r,
                         _stream(stream)))
     return complex(r[0], r[1])
+
+
+def bs_noalloc_setup():
+    _check(_lib.bs_noalloc_setup())
+
+
+def bs_noalloc_max_dim() -> int:
+    return int(_lib.bs_noalloc_max_dim())
+
+
+def bs_vdot_noalloc(a, b, result, stream=None):
+    """result (complex128 CUDA tensor of one element) <- <a|b>; allocates nothing, does not synchronise."""
+    n = a.numel()
+    _check(_lib.bs_vdot_noalloc(_dev_ptr(a, n, "a"), _dev_ptr(b, n, "b"), n, _dev_ptr(result, 1, "result"),
+                                _stream(stream)))
+    return result
 
 
 def bs_apply_pauli_rotations(generators: Op, sector: Sector, thetas, psi, stream=None):
