@@ -353,7 +353,7 @@ std::vector<u32> subsets(int n, int k) {
 
 bs_kres::~bs_kres() { delete rp; }
 
-int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st, bs_kres** out) {
+int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st, bs_kres** out, bool allow_xa0) {
     *out = nullptr;
     if (getenv("BS_NO_KRES")) return BS_OK;   // test hook (include/bs.h "Environment")
     const int n = S->n_orb, Nb = S->n_beta;
@@ -380,11 +380,12 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
     const int min_hops = getenv("BS_KRES_MIN") ? atoi(getenv("BS_KRES_MIN")) : 8;
     std::map<u32, int> n_hops;
     for (auto& g : groups)
-        if (g.xa != 0 && jw_hop(g)) ++n_hops[g.xa];
+        if ((g.xa != 0 || allow_xa0) && jw_hop(g)) ++n_hops[g.xa];
     std::vector<HostGroup> mine, rest;
     for (auto& g : groups) {
         auto f = n_hops.find(g.xa);
-        const bool take = g.xa != 0 && f != n_hops.end() && f->second >= min_hops && (jw_hop(g) || absorbable(g));
+        const bool take = f != n_hops.end() && f->second >= min_hops &&
+                          ((g.xa != 0 && (jw_hop(g) || absorbable(g))) || (g.xa == 0 && allow_xa0 && jw_hop(g)));
         (take ? mine : rest).push_back(g);
     }
     if (mine.empty()) return BS_OK;

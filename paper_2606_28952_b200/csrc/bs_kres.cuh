@@ -82,5 +82,7 @@ struct bs_kres {
 struct bs_sector;
 // Splits the kres-able groups off `groups` (they are removed from it) and builds the tables; *out stays null when
 // nothing qualifies or a limit is hit (the groups then remain in `groups`).
-int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st, bs_kres** out);
+// allow_xa0: also take single-key JW hops under the identity alpha move (the alpha-spectator part of beta single hops,
+// split off by the plan builder); never the x = 0 diagonal group.
+int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st, bs_kres** out, bool allow_xa0 = false);
 int bs_kres_apply(bs_kres* K, const double2* psi, i64 row_lo, i64 row_hi, cudaStream_t st);

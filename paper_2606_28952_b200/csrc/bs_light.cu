@@ -321,6 +321,7 @@ int bs_light_build(bs_rowplan* R, cudaStream_t st) {
     if (getenv("BS_NO_LIGHT")) return BS_OK;
     const RowPlanDev& P = R->dev;
     const i64 Da = P.A.D, Db = P.B.D;
+    if (R->has_cdiag) return BS_OK;   // k_light does not read the per-column diagonal table
     if (!R->real_w || Db > 4094 || Db < 64 || R->h_hdrs.empty() || R->h_xa[0] != 0) return BS_OK;
     const XaHdr& h0 = R->h_hdrs[0];
     const bool listed = h0.item_split < h0.item1;

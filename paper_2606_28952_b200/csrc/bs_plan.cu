@@ -54,22 +54,67 @@ void build_row_plans(bs_plan* P, const std::vector<HostGroup>& groups, bs_sector
     for (auto& g : groups) nB += (g.xa == 0 && g.xb != 0);
     const bool transposed_b = nB > 64 && !(force && std::string(force) == "v2inrow");
     std::vector<HostGroup> main_g, t_g;
+    auto to_transposed = [&](u32 xb, const std::vector<HostStr>& strs) {
+        HostGroup t;
+        t.xa = xb;
+        t.xb = 0;
+        for (auto& s : strs) t.s.push_back(HostStr{s.zb, s.za, s.re, s.im});
+        std::stable_sort(t.s.begin(), t.s.end(), [](const HostStr& a, const HostStr& b) {
+            return a.zb < b.zb || (a.zb == b.zb && a.za < b.za);
+        });
+        t_g.push_back(std::move(t));
+    };
+    // Beta single hops (x_a = 0, x_b = {r, s}) of a two-body Hamiltonian carry two kinds of strings: the JW chain between
+    // r and s, alone or with one ALPHA Z (alpha spectator densities: F depends on t_a, not on the other beta electrons),
+    // and the chain with one more BETA Z and no alpha Z (beta spectators: F depends on t_b only).  The first kind is an
+    // alpha-beta coupling with the identity as its alpha move: it joins the K-resolved kernel as one more entry per row
+    // (G[s][r] = A_rs(t_a)).  The second kind is the same sparse matrix for every alpha row: on the transposed problem it
+    // is a plain row axpy with one scalar per (t_b, hop).  Without the split the group is a 1 + n-key item per non-zero.
+    const bool hop_split = transposed_b && !getenv("BS_NO_KRES") && !getenv("BS_NO_HOPSPLIT");
+    bool any_split = false;
     for (auto& g : groups) {
         if (transposed_b && g.xa == 0 && g.xb != 0) {
-            HostGroup t;
-            t.xa = g.xb;
-            t.xb = 0;
-            for (auto& s : g.s) t.s.push_back(HostStr{s.zb, s.za, s.re, s.im});
-            std::stable_sort(t.s.begin(), t.s.end(), [](const HostStr& a, const HostStr& b) {
-                return a.zb < b.zb || (a.zb == b.zb && a.za < b.za);
-            });
-            t_g.push_back(std::move(t));
+            bool done = false;
+            if (hop_split && __builtin_popcount(g.xb) == 2) {
+                const int lo = __builtin_ctz(g.xb), hi = 31 - __builtin_clz(g.xb);
+                const u32 between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
+                std::vector<HostStr> part_a, part_b;
+                bool ok = true;
+                u32 zb_chain = 0;
+                bool have_chain = false;
+                for (auto& st_ : g.s)
+                    if ((st_.zb & ~g.xb) == between && (!have_chain || st_.zb == zb_chain)) {
+                        zb_chain = st_.zb;
+                        have_chain = true;
+                    }
+                for (auto& st_ : g.s) {
+                    if (have_chain && st_.zb == zb_chain) part_a.push_back(st_);
+                    else {
+                        part_b.push_back(st_);
+                        ok &= st_.za == 0;
+                    }
+                    ok &= st_.im == 0.0;
+                }
+                if (ok && have_chain && !part_a.empty()) {
+                    HostGroup a;
+                    a.xa = 0;
+                    a.xb = g.xb;
+                    a.s = part_a;
+                    main_g.push_back(std::move(a));
+                    if (!part_b.empty()) to_transposed(g.xb, part_b);
+                    done = any_split = true;
+                }
+            }
+            if (!done) to_transposed(g.xb, g.s);
         } else main_g.push_back(g);
     }
+    std::stable_sort(main_g.begin(), main_g.end(), [](const HostGroup& a, const HostGroup& b) {
+        return a.xa < b.xa || (a.xa == b.xa && a.xb < b.xb);
+    });
     std::stable_sort(t_g.begin(), t_g.end(), [](const HostGroup& a, const HostGroup& b) { return a.xa < b.xa; });
     // alpha-beta groups with JW chains: K-resolved kernel (bs_kres.cuh); what it takes leaves main_g
     bs_kres* kres = nullptr;
-    if (bs_kres_build(main_g, S, st, &kres) != BS_OK) {
+    if (bs_kres_build(main_g, S, st, &kres, any_split) != BS_OK) {
         cudaGetLastError();
         kres = nullptr;
         P->rows_fallback = 1;

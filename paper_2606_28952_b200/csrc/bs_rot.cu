@@ -507,8 +507,10 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                                                 thetas[j], sc1, psi);
         BS_COUNT_LAUNCH(1);
     };
-    const bool batching = RR && RR->coff.back() > 0 && !getenv("BS_ROT_PER_LAUNCH");
-    const bool in_place = getenv("BS_ROT_IN_PLACE") != nullptr;   // test hook: cells in place (L2) even when they fit shared memory
+    // test hooks, read once per process (never on a launch path)
+    static const bool env_per_launch = getenv("BS_ROT_PER_LAUNCH") != nullptr;
+    static const bool in_place = getenv("BS_ROT_IN_PLACE") != nullptr;   // cells in place (L2) even when they fit shared memory
+    const bool batching = RR && RR->coff.back() > 0 && !env_per_launch;
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
         const u64 mask_a = (u64(1) << s->n_orb) - 1;

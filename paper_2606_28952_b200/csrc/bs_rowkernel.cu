@@ -40,6 +40,8 @@ struct VT<true> {
         acc.y += f * a.y;
     }
     static __device__ __forceinline__ double from(double2 w) { return w.x; }
+    static __device__ __forceinline__ void add_real(double& f, double v) { f += v; }
+    static __device__ __forceinline__ double shfl_add(double f, int o) { return f + __shfl_xor_sync(0xffffffffu, f, o); }
 };
 template <>
 struct VT<false> {
@@ -56,6 +58,10 @@ struct VT<false> {
         acc.y += f.x * a.y + f.y * a.x;
     }
     static __device__ __forceinline__ double2 from(double2 w) { return w; }
+    static __device__ __forceinline__ void add_real(double2& f, double v) { f.x += v; }
+    static __device__ __forceinline__ double2 shfl_add(double2 f, int o) {
+        return make_double2(f.x + __shfl_xor_sync(0xffffffffu, f.x, o), f.y + __shfl_xor_sync(0xffffffffu, f.y, o));
+    }
 };
 
 // CPT packed u16 table entries of one thread (the table is stored thread-blocked, see bs_rowplan.cu)
@@ -126,14 +132,18 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
                 if (STAGED) a[c] = (!WINDOWED || (col[c] - w0) < wn) ? srow[col[c] - w0] : make_double2(0.0, 0.0);
                 else a[c] = __ldg(srcp + col[c]);
             }
-            if (it.z == 1) {
+            if (it.z == 1 && !(it.w & 2u)) {
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) V::fma(acc[c], f0, 0u, a[c]);
             } else {
                 vt f[CPT];
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) f[c] = f0;
-                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w, tb);
+                if (it.w & 2u) {   // row-independent (real) part of the diagonal group, tabulated per column
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) V::add_real(f[c], __ldg(P.cdiag + col[c]));
+                }
+                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w & 1u, tb);
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) V::fma(acc[c], f[c], 0u, a[c]);
             }
@@ -152,7 +162,7 @@ __device__ __forceinline__ void process_entry(const RowPlanDev& P, const uint4* 
                 vt f[CPT];
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) f[c] = f0;
-                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w, tb);
+                multi_key<REALW, CPT>(f, v, P.key_dz + it.y, it.z, it.w & 1u, tb);
 #pragma unroll
                 for (int c = 0; c < CPT; ++c) {
                     const u32 src = en16[c] & 0x7FFFu;
@@ -290,6 +300,17 @@ k_rows(const RowPlanDev P, const double2* __restrict__ psi, double2* __restrict_
                     const uint4 en = __ldg(P.row_ent + j);
                     const u32 key0 = __ldg(reinterpret_cast<const u32*>(P.xa_hdr + en.x) + 2);
                     const u32 nk = en.w & 0x3FFFFFFFu;
+                    if (nk == 1 && !listed) {
+                        // one key with many strings (e.g. a beta hop's beta-spectator sum on the transposed problem): the
+                        // lanes share the strings, fixed-order butterfly
+                        vt f = V::zero();
+                        const u32 s1 = __ldg(P.key_s0 + key0 + 1);
+                        for (u32 s = __ldg(P.key_s0 + key0) + lane; s < s1; s += 32)
+                            V::addflip(f, V::from(__ldg(P.s_w + s)), (u32)__popc(__ldg(P.s_za + s) & ta) & 1u);
+                        for (int o = 16; o > 0; o >>= 1) f = V::shfl_add(f, o);
+                        if (lane == 0) sV[en.z - kbase] = f;
+                        continue;
+                    }
                     for (u32 k = lane; k < nk; k += 32) {
                         vt f = V::zero();
                         const u32 s1 = __ldg(P.key_s0 + key0 + k + 1);

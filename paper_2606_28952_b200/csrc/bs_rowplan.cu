@@ -48,6 +48,18 @@ __global__ void k_list_build(const unsigned short* __restrict__ T, i64 tstride, 
     else for (; j < l_max; ++j) L[(i64)j * tstride + slot] = pad_src | ((u32)n_listed << 16);
 }
 
+// per-column constant of the diagonal group: cdiag[col] = sum_s w_s (-1)^{popc(zb_s & t_b)} over its strings whose weight
+// does not depend on the row (z_a = 0: pure column-spin Z strings, e.g. the C(n,2) Z_q Z_q' pairs of a two-body H)
+__global__ void k_cdiag(SpinTab B, const u32* __restrict__ zb, const double* __restrict__ w, int n,
+                        double* __restrict__ cdiag) {
+    const i64 col = blockIdx.x * (i64)blockDim.x + threadIdx.x;
+    if (col >= B.D) return;
+    const u32 tb = B.str[col];
+    double f = 0.0;
+    for (int s = 0; s < n; ++s) f += (__popc(__ldg(zb + s) & tb) & 1) ? -__ldg(w + s) : __ldg(w + s);
+    cdiag[col] = f;
+}
+
 __global__ void k_row_count2(SpinTab A, const u32* __restrict__ xa, int n_xa, int* __restrict__ cnt) {
     i64 r = blockIdx.x * (i64)blockDim.x + threadIdx.x;
     if (r >= A.D) return;
@@ -113,6 +125,40 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
         return la < lb;
     });
     BS_REQUIRE(Db <= 32767, BS_ERR_ARG, "row plan: column space too large for u16 tables");
+    // Diagonal group (x = 0): keys whose strings all have z_a = 0 and z_b != 0 carry a row-independent weight; when they
+    // are many (two-body H: the C(n,2) pairs Z_q Z_q' of the column spin, 378 of 407 keys at configs[4]) their sum is a
+    // per-COLUMN constant, tabulated once (k_cdiag) and added by the kernel; the item keeps its row-dependent keys, which
+    // are then single-bit masks (bit test instead of POPC).  Real weights only; BS_NO_CDIAG (test hook) switches it off.
+    std::vector<u32> cd_zb;
+    std::vector<double> cd_w;
+    int cdiag_group = -1;
+    if (with_tables && !getenv("BS_NO_CDIAG"))
+        for (size_t g = 0; g < groups.size(); ++g) {
+            HostGroup& hg = groups[g];
+            if (hg.xa != 0 || hg.xb != 0 || hg.s.front().zb != 0) continue;
+            bool real = true;
+            for (auto& st_ : hg.s) real &= st_.im == 0.0;
+            if (!real) break;
+            std::map<u32, bool> row_indep;   // per zb key: every string has z_a = 0
+            for (auto& st_ : hg.s) {
+                auto f = row_indep.find(st_.zb);
+                if (f == row_indep.end()) row_indep[st_.zb] = st_.za == 0;
+                else f->second = f->second && st_.za == 0;
+            }
+            int n_const = 0;
+            for (auto& kv : row_indep) n_const += kv.first != 0 && kv.second;
+            if (n_const < 8) break;
+            std::vector<HostStr> keep;
+            for (auto& st_ : hg.s) {
+                if (st_.zb != 0 && row_indep[st_.zb]) {
+                    cd_zb.push_back(st_.zb);
+                    cd_w.push_back(st_.re);
+                } else keep.push_back(st_);
+            }
+            hg.s.swap(keep);
+            cdiag_group = (int)g;
+            break;
+        }
     std::vector<u32> xa_list, key_dz, key_s0, s_za;
     std::vector<XaHdr> hdrs;
     std::vector<RowItem> items;
@@ -155,6 +201,7 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
             if (hg.s[k].im != 0.0) real_w = false;
         }
         it.nkeys = (u32)key_dz.size() - it.key0;
+        if ((int)g == cdiag_group) it.single |= 2u;   // the kernel adds cdiag[col]
         if (hg.xb == 0 && zb0 == 0) it.tkey = kTkeyIdent;
         else {
             auto key = std::make_pair(hg.xb, zb0);
@@ -267,6 +314,17 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
                                           R->d_ttab.p + k0 * R->tstride);
         BS_COUNT_LAUNCH(1);
     }
+    R->has_cdiag = cdiag_group >= 0;
+    if (R->has_cdiag) {
+        DevBuf<u32> d_zb;
+        DevBuf<double> d_w;
+        BS_CUDA(d_zb.upload(cd_zb, st));
+        BS_CUDA(d_w.upload(cd_w, st));
+        BS_CUDA(R->d_cdiag.alloc(Db));
+        k_cdiag<<<(unsigned)((Db + 255) / 256), 256, 0, st>>>(B, d_zb.p, d_w.p, (int)cd_zb.size(), R->d_cdiag.p);
+        BS_COUNT_LAUNCH(1);
+        BS_CUDA(cudaStreamSynchronize(st));   // the uploads' sources and device buffers die here
+    }
     // column list: compaction of the listed tables over table ids
     R->n_listed = n_listed;
     R->h_hdrs = hdrs;
@@ -364,5 +422,6 @@ int bs_rowplan_build(bs_rowplan* R, const std::vector<HostGroup>& groups_in, con
     d.l_woff = R->l_split ? R->d_lwoff.p : nullptr;
     d.l_nchunks = R->n_chunks;
     d.n_listed = n_listed;
+    d.cdiag = R->has_cdiag ? R->d_cdiag.p : nullptr;
     return BS_OK;
 }

@@ -29,7 +29,7 @@ struct __align__(16) RowItem {
     u32 tkey;   // column table id or kTkeyIdent
     u32 key0;   // first key (global index)
     u32 nkeys;  // >= 1
-    u32 single; // 1: every dz of keys 1.. has exactly one bit (bit test instead of POPC)
+    u32 single; // bit 0: every dz of keys 1.. has exactly one bit (bit test instead of POPC); bit 1: add cdiag[col]
 };
 
 // device view handed to the kernel by value
@@ -57,6 +57,7 @@ struct RowPlanDev {
     const int* l_woff;          // nullptr: one list for all windows (entries carry a window test); then per (window, chunk) slot counts
     int l_nchunks;
     int l_max, n_listed;
+    const double* cdiag;        // [Db] row-independent part of the diagonal group (items with single & 2), or nullptr
 };
 
 struct bs_rowplan {
@@ -71,6 +72,8 @@ struct bs_rowplan {
     DevBuf<double2> d_s_w;
     DevBuf<unsigned short> d_ttab;
     DevBuf<u32> d_ltab;
+    DevBuf<double> d_cdiag;
+    bool has_cdiag = false;
     DevBuf<int> d_lwoff;
     bool l_split = false;
     int l_max = 0, n_listed = 0;
