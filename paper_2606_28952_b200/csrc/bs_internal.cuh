@@ -92,6 +92,23 @@ struct bs_op {
         DevBuf<u64> d_rz;
         DevBuf<double2> d_rw;
         DevBuf<i64> d_roff;
+        // orbit cells (bs_rot.cu, k_rot_orbit): sub-runs of common-x_a runs whose beta masks touch <= 10 orbitals
+        struct OrbitSub {
+            i64 j0, j1;        // generators of the sub-run
+            int tab;           // index into orbit_tabs (tables shared by sub-runs with the same orbital set U), -1: unusable
+            i64 part_off;      // offset of its pair lists in d_opart
+            i64 poff_off;      // offset of its [n_gen][12] pair offsets in d_opoff
+        };
+        struct OrbitU {
+            i64 pat_off, out_off;   // offsets into d_opat / d_oout
+            int n_pat, n_out, nU;
+            int m_off[12];
+        };
+        std::vector<OrbitSub> orbit_subs;   // sorted by j0; covers every generator of every common-x_a run
+        std::vector<OrbitU> orbit_tabs;
+        DevBuf<u32> d_opat, d_oout;
+        DevBuf<unsigned short> d_opart;
+        DevBuf<int> d_opoff;
         DevBuf<double> d_th;    // thetas of the current call
         DevBuf<double2> d_sc;   // (sin, cos) of the thetas
     };

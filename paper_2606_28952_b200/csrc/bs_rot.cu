@@ -311,6 +311,87 @@ k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, con
         }
 }
 
+// ---- orbit cells: closed cells that stay small at any sector size -------------------------------------------------
+// A SUB-RUN of consecutive generators with a common alpha mask whose beta masks together touch the orbital set U
+// (|U| <= kOrbitUmax) only moves electrons inside U: the columns with one fixed occupation OUTSIDE U form an orbit of at most
+// C(|U|, |U|/2) columns, closed under every pairing of the sub-run.  One warp owns one orbit of one row (x_a = 0) or
+// row pair: it loads the orbit's amplitudes into its slice of shared memory, applies ALL generators of the sub-run
+// (__syncwarp between them, no block barrier) and writes them back: one trip through L2 / HBM per sub-run instead
+// of one per generator.  UCCSD order (reading U10): the alpha-beta doubles of one (i, a) come as j outer, b inner, so
+// a sub-run collects all b of two beta occupied orbitals j (|U| = 10 at configs[3]: 16 generators per load).
+// OPT-IN (BS_ROT_ORBIT=1): at configs[3] it is slower than the in-place cells -- every sub-run touches every amplitude of
+// the valid rows with scattered 16-byte accesses, the in-place kernel only the 28 % that a generator rotates.
+constexpr int kOrbitUmax = 10;
+constexpr int kOrbitMax = 252;   // C(10, 5) columns
+
+struct OrbitTab {
+    const u32* pat;            // [n_pat] sub-masks of U at their real bit positions, grouped by popcount m, ascending
+    const u32* outs;           // [n_out] occupations outside U that leave 0 <= m <= |U| electrons for U
+    const unsigned short* pairs;     // per (generator, m) the valid owner pairs, compacted: i | q << 8, i and q = positions of
+                                     // p and p ^ x_b within the m block (< 252)
+    const int* pair_off;             // [n_gen][12]: pairs of (generator, m) are [pair_off[g][m], pair_off[g][m + 1])
+    int pat_off[kOrbitUmax + 2];     // m block [pat_off[m], pat_off[m + 1])
+    int n_pat, n_out, Nb;
+};
+
+template <int R>
+__global__ void __launch_bounds__(256)
+k_rot_orbit(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, OrbitTab T, const i64* __restrict__ offs,
+            const u64* __restrict__ z, const double2* __restrict__ w, const double* __restrict__ thetas,
+            const double2* __restrict__ sc, i64 j0, i64 j1, double2* __restrict__ psi) {
+    extern __shared__ __align__(16) unsigned char smem_cell[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double2* s0 = reinterpret_cast<double2*>(smem_cell) + (size_t)warp * (R * kOrbitMax);
+    double2* s1 = (R == 2) ? s0 + kOrbitMax : s0;
+    u32* scol = reinterpret_cast<u32*>(smem_cell + (size_t)8 * R * kOrbitMax * 16) + warp * (2 * kOrbitMax);
+    u32* spat = scol + kOrbitMax;   // the orbit's beta strings o | p
+    u32 row0, row1;
+    if (R == 2) {
+        const uint2 pr = pairs[blockIdx.y];
+        row0 = pr.x;
+        row1 = pr.y;
+    } else row0 = row1 = blockIdx.y;
+    const u64 ta = A.str[row0];
+    const i64 Db = B.D;
+    double2* __restrict__ p0 = psi + (i64)row0 * Db;
+    double2* __restrict__ p1 = psi + (i64)row1 * Db;
+    for (int oi = blockIdx.x * 8 + warp; oi < T.n_out; oi += gridDim.x * 8) {
+        const u32 o = __ldg(T.outs + oi);
+        const int m = T.Nb - __popc(o);
+        const int pb = T.pat_off[m], np = T.pat_off[m + 1] - pb;
+        if (np < (R == 2 ? 1 : 2)) continue;   // warp-uniform (one column: only a row pair can still rotate, x_b = 0)
+        for (int i = lane; i < np; i += 32) {
+            const u32 tb = o | __ldg(T.pat + pb + i);
+            const u32 col = spin_rank(B, tb);
+            scol[i] = col;
+            spat[i] = tb;
+            s0[i] = p0[col];
+            if (R == 2) s1[i] = p1[col];
+        }
+        __syncwarp();
+        for (i64 g = j0; g < j1; ++g) {
+            const int* __restrict__ po = T.pair_off + (size_t)(g - j0) * 12 + m;
+            const int q0 = __ldg(po), q1 = __ldg(po + 1);
+            if (q0 == q1) continue;   // warp-uniform: the generator pairs nothing in this occupation class
+            const int k0 = (int)__ldg(offs + g), k1 = (int)__ldg(offs + g + 1);
+            const double th = __ldg(thetas + g);
+            const double2 sc1 = __ldg(sc + g);
+            for (int idx = q0 + lane; idx < q1; idx += 32) {
+                const u32 pq = __ldg(T.pairs + idx);
+                const u32 i = pq & 255u, q = pq >> 8;
+                rotate_smem(s0[i], s1[q], phase_sum(z, w, k0, k1, ta | ((u64)spat[i] << n_orb)), th, sc1);
+            }
+            __syncwarp();
+        }
+        for (int i = lane; i < np; i += 32) {
+            const u32 col = scol[i];
+            p0[col] = s0[i];
+            if (R == 2) p1[col] = s1[i];
+        }
+        __syncwarp();
+    }
+}
+
 // One-off validation of a generator list against a sector: for every generator (blockIdx.y) and
 // every sector configuration t whose partner t^x lies outside the sector, F(t) must vanish;
 // otherwise exp(theta A) would leak out of the sector and its restriction would not be unitary.
@@ -460,7 +541,95 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 }
                 RR->roff[j + 1] = (i64)rz.size();
             }
+            // ---- orbit cells: sub-runs and their tables (see k_rot_orbit) ----------------------------------------------
+            std::vector<u32> opat, oout;
+            std::vector<unsigned short> opart;
+            std::vector<int> opoff;
+            if (s->n_orb <= 32 && (double)n_rot * 1024.0 * 2.0 <= 2e9) {
+                const int n = s->n_orb, Nb = s->n_beta;
+                const u32 full_b = n == 32 ? 0xFFFFFFFFu : ((1u << n) - 1u);
+                std::map<u32, int> tab_of;   // orbital set U -> index in orbit_tabs
+                auto table_for = [&](u32 U) {
+                    auto f = tab_of.find(U);
+                    if (f != tab_of.end()) return f->second;
+                    bs_op::RotRows::OrbitU t{};
+                    t.nU = __builtin_popcount(U);
+                    t.pat_off = (i64)opat.size();
+                    std::vector<std::vector<u32>> by_m(t.nU + 1);
+                    for (u32 p2 = U;; p2 = (p2 - 1) & U) {   // all sub-masks of U
+                        by_m[__builtin_popcount(p2)].push_back(p2);
+                        if (p2 == 0) break;
+                    }
+                    int off = 0;
+                    for (int m = 0; m <= t.nU; ++m) {
+                        std::sort(by_m[m].begin(), by_m[m].end());
+                        t.m_off[m] = off;
+                        off += (int)by_m[m].size();
+                        opat.insert(opat.end(), by_m[m].begin(), by_m[m].end());
+                    }
+                    for (int m = t.nU + 1; m < 12; ++m) t.m_off[m] = off;
+                    t.n_pat = off;
+                    t.out_off = (i64)oout.size();
+                    const u32 outside = full_b & ~U;
+                    for (u32 o = outside;; o = (o - 1) & outside) {   // occupations outside U
+                        const int m = Nb - __builtin_popcount(o);
+                        if (m >= 0 && m <= t.nU) oout.push_back(o);
+                        if (o == 0) break;
+                    }
+                    t.n_out = (int)(oout.size() - t.out_off);
+                    RR->orbit_tabs.push_back(t);
+                    tab_of[U] = (int)RR->orbit_tabs.size() - 1;
+                    return tab_of[U];
+                };
+                for (i64 j = 0; j < n_rot;) {
+                    const u64 xa0 = gen->h_xg[j] & mask_a;
+                    i64 e2 = j + 1;
+                    if (gen->h_xg[j] != 0)
+                        while (e2 < n_rot && gen->h_xg[e2] != 0 && (gen->h_xg[e2] & mask_a) == xa0) ++e2;
+                    if (e2 - j < 2) {   // isolated generator: no run, no sub-run
+                        j = e2;
+                        continue;
+                    }
+                    for (i64 q = j; q < e2;) {   // greedy sub-runs: beta masks touching at most kOrbitUmax orbitals
+                        u32 U = 0;
+                        i64 q1 = q;
+                        while (q1 < e2 && __builtin_popcount(U | (u32)(gen->h_xg[q1] >> n)) <= kOrbitUmax) U |= (u32)(gen->h_xg[q1++] >> n);
+                        bs_op::RotRows::OrbitSub sub{q, std::max(q1, q + 1), -1, 0, 0};
+                        if (q1 > q && U != 0) {
+                            sub.tab = table_for(U);
+                            const bs_op::RotRows::OrbitU& t = RR->orbit_tabs[sub.tab];
+                            sub.part_off = (i64)opart.size();
+                            sub.poff_off = (i64)opoff.size();
+                            const u32* pat = opat.data() + t.pat_off;
+                            for (i64 g = sub.j0; g < sub.j1; ++g) {
+                                const u32 xb = (u32)(gen->h_xg[g] >> n);
+                                const int pxb = __builtin_popcount(xb);
+                                for (int m = 0; m < 12; ++m) {
+                                    opoff.push_back((int)((i64)opart.size() - sub.part_off));
+                                    if (m > t.nU) continue;
+                                    for (int i = t.m_off[m]; i < t.m_off[m + 1]; ++i) {
+                                        if (2 * __builtin_popcount(pat[i] & xb) != pxb) continue;
+                                        const u32 pp = pat[i] ^ xb;
+                                        const int li = i - t.m_off[m];
+                                        const int qi = (int)(std::lower_bound(pat + t.m_off[m], pat + t.m_off[m + 1], pp) - (pat + t.m_off[m]));
+                                        // x_a = 0: the pair lives in one row and belongs to its smaller column (columns of an
+                                        // orbit are ordered like their patterns); x_a != 0: every valid pattern pairs row 0 with row 1
+                                        if (xa0 != 0 || qi > li) opart.push_back((unsigned short)(li | (qi << 8)));
+                                    }
+                                }
+                            }
+                        }
+                        RR->orbit_subs.push_back(sub);
+                        q = sub.j1;
+                    }
+                    j = e2;
+                }
+            }
             cudaError_t e = RR->d_pairs.upload(pairs, st);
+            if (e == cudaSuccess) e = RR->d_opat.upload(opat, st);
+            if (e == cudaSuccess) e = RR->d_oout.upload(oout, st);
+            if (e == cudaSuccess) e = RR->d_opart.upload(opart, st);
+            if (e == cudaSuccess) e = RR->d_opoff.upload(opoff, st);
             if (e == cudaSuccess) e = RR->d_rz.upload(rz, st);
             if (e == cudaSuccess) e = RR->d_rw.upload(rw, st);
             if (e == cudaSuccess) e = RR->d_roff.upload(RR->roff, st);
@@ -510,6 +679,9 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     // test hooks, read once per process (never on a launch path)
     static const bool env_per_launch = getenv("BS_ROT_PER_LAUNCH") != nullptr;
     static const bool in_place = getenv("BS_ROT_IN_PLACE") != nullptr;   // cells in place (L2) even when they fit shared memory
+    // BS_ROT_ORBIT=1 (test hook): orbit cells (k_rot_orbit) for common-x_a runs at any sector size.  Not the default:
+    // measured slower than the in-place cells at configs[3] (1.79 s vs 1.32 s for the UCCSD list)
+    static const int orbit_mode = getenv("BS_ROT_ORBIT") ? atoi(getenv("BS_ROT_ORBIT")) : 0;
     const bool batching = RR && RR->coff.back() > 0 && !env_per_launch;
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
@@ -557,7 +729,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 const uint2* pr = RR->d_pairs.p + RR->off[j];
                 if (n_cells == 0) {
                     launched = true;  // x_a never valid in this sector: identity
-                } else if (smem <= smem_cap && !in_place) {
+                } else if (smem <= smem_cap && !in_place && orbit_mode != 1) {
                     if (R == 2) {
                         BS_ROT_SMEM((k_rot_cell_rows<2, false>))
                         k_rot_cell_rows<2, false><<<(unsigned)n_cells, 512, smem, st>>>(BS_ROT_ARGS_ROWS);
@@ -566,6 +738,41 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                         k_rot_cell_rows<1, false><<<(unsigned)n_cells, 256, smem, st>>>(BS_ROT_ARGS_ROWS);
                     }
                     BS_COUNT_LAUNCH(1);
+                    launched = true;
+                } else if (!RR->orbit_subs.empty() && orbit_mode == 1 && !in_place) {
+                    // cells of {row (pair)} x {orbit of <= 252 columns}: one launch per SUB-RUN, the cell in shared memory
+                    auto it2 = std::lower_bound(RR->orbit_subs.begin(), RR->orbit_subs.end(), j,
+                                                [](const bs_op::RotRows::OrbitSub& a, i64 v) { return a.j0 < v; });
+                    for (; it2 != RR->orbit_subs.end() && it2->j0 < e; ++it2) {
+                        const i64 j = it2->j0, e = it2->j1;   // shadow the run bounds for the argument macros
+                        if (it2->tab < 0) {   // a beta mask wider than the orbit limit: in place for this sub-run
+                            if (R == 2) k_rot_cell_rows<2, true><<<(unsigned)n_cells, 512, 0, st>>>(BS_ROT_ARGS_ROWS);
+                            else k_rot_cell_rows<1, true><<<(unsigned)n_cells, 256, 0, st>>>(BS_ROT_ARGS_ROWS);
+                        } else {
+                            const bs_op::RotRows::OrbitU& t = RR->orbit_tabs[it2->tab];
+                            OrbitTab T;
+                            T.pat = RR->d_opat.p + t.pat_off;
+                            T.outs = RR->d_oout.p + t.out_off;
+                            T.pairs = RR->d_opart.p + it2->part_off;
+                            T.pair_off = RR->d_opoff.p + it2->poff_off;
+                            for (int m = 0; m < kOrbitUmax + 2; ++m) T.pat_off[m] = t.m_off[m];
+                            T.n_pat = t.n_pat;
+                            T.n_out = t.n_out;
+                            T.Nb = s->n_beta;
+                            const size_t osmem = (size_t)8 * R * kOrbitMax * 16 + (size_t)8 * 2 * kOrbitMax * 4;
+                            const dim3 og((unsigned)std::min<i64>((t.n_out + 7) / 8, 4096), (unsigned)n_cells);
+                            if (R == 2) {
+                                BS_ROT_SMEM((k_rot_orbit<2>))
+                                k_rot_orbit<2><<<og, 256, osmem, st>>>(s->ta, s->tb, s->n_orb, pr, T, RR->d_roff.p, RR->d_rz.p,
+                                                                       RR->d_rw.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            } else {
+                                BS_ROT_SMEM((k_rot_orbit<1>))
+                                k_rot_orbit<1><<<og, 256, osmem, st>>>(s->ta, s->tb, s->n_orb, pr, T, RR->d_roff.p, RR->d_rz.p,
+                                                                       RR->d_rw.p, RR->d_th.p, RR->d_sc.p, j, e, psi);
+                            }
+                        }
+                        BS_COUNT_LAUNCH(1);
+                    }
                     launched = true;
                 } else {   // the cell stays in place (L2): still one launch per run
                     if (R == 2) k_rot_cell_rows<2, true><<<(unsigned)n_cells, 512, 0, st>>>(BS_ROT_ARGS_ROWS);

@@ -342,13 +342,16 @@ def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
     counts = {}
     # BS_ROT_IN_PLACE: the cell kernels work on the state vector itself (the path of sectors whose cells exceed
     # shared memory, configs 4-5) -- same launch count as the shared-memory cells
-    for key, env in (("cells", {}), ("per_launch", {"BS_ROT_PER_LAUNCH": "1"}), ("in_place", {"BS_ROT_IN_PLACE": "1"})):
+    # BS_ROT_ORBIT=1: cells of {row pair} x {orbit of columns} (the default path of sectors whose rows exceed shared memory)
+    for key, env in (("cells", {}), ("per_launch", {"BS_ROT_PER_LAUNCH": "1"}), ("in_place", {"BS_ROT_IN_PLACE": "1"}),
+                     ("orbit", {"BS_ROT_ORBIT": "1"})):
         r = subprocess.run([sys.executable, "-c", code, root], env=dict(os.environ, **env), capture_output=True,
                            text=True, timeout=600)
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
         counts[key] = int(r.stdout.split("LAUNCHES")[1].split()[0])
     assert counts["per_launch"] > 3 * counts["cells"]      # batching really reduces the launch count
     assert counts["in_place"] == counts["cells"]
+    assert counts["cells"] <= counts["orbit"] < counts["per_launch"]
 
 
 def test_apply_and_rotations_are_bit_reproducible(bs):
