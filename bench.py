@@ -209,6 +209,35 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf, with_cpu:
     return ent
 
 
+def tfim_entry(bs, torch, peak_gbs: float, flush_buf, n_qubits: int = 20):
+    """NEXT-2: the paper's dynamics model in the FULL 2^N space (Eq. 40),
+    a number-non-conserving operator: plain bs_apply / bs_expect through the full-space kernel (k_apply_full)."""
+    x, z, c = si.tfim_terms(n_qubits)
+    op = bs.bs_group_xmask(x, z, c, n_qubits, 0.0)
+    sec = bs.bs_sector_build(n_qubits)
+    D = 1 << n_qubits
+    psi = torch.from_numpy(si.random_state(D, 40 + n_qubits)).cuda()
+    out = torch.empty_like(psi)
+    bs.bs_apply(op, sec, psi, out)
+    times = []
+    for _ in range(10):
+        flush_buf.zero_()                                  # 2 x 16 MB would sit in the 126 MB L2
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        bs.bs_apply(op, sec, psi, out)
+        b.record()
+        torch.cuda.synchronize()
+        times.append(a.elapsed_time(b))
+    ms = _median(times)
+    e = bs.bs_expect(op, sec, psi)
+    bytes_alg = 32 * D + table_bytes(op)
+    return {"n_qubits": n_qubits, "dim": D, "groups": op.n_groups, "strings": op.n_terms, "space": "full 2^N",
+            "plan": bs.bs_plan_describe(op, sec), "apply_ms": ms, "applies_per_s": 1e3 / ms,
+            "l2_flush_between_reps": True, "hbm_gbs_algorithmic": bytes_alg / ms / 1e6,
+            "hbm_frac_of_measured_peak": bytes_alg / ms / 1e6 / peak_gbs, "energy": e.real,
+            "gathers_per_target": op.n_groups}
+
+
 def cpu_baseline(name: str, max_seconds: float = 30.0):
     """The oracle's Eq. 27 gather (OpenMP over target rows, as it stands) on this host's cores, on a bounded sample.
     Small sectors: orc_apply_grouped on an alpha-row slab, scaled linearly in rows.  configs 4-5: the per-row beta
@@ -412,6 +441,7 @@ def run_ours(args):
             flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
             line["per_config"] = {n: per_config_entry(n, bs, torch, peak_gbs, flush_buf, not args.no_cpu_baseline)
                                   for n in want}
+            line["per_config"]["tfim20_full_space"] = tfim_entry(bs, torch, peak_gbs, flush_buf)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(name)
         print(json.dumps(line), flush=True)

@@ -124,3 +124,14 @@ def uccsd_excitations(n_orb: int, n_alpha: int, n_beta: int):
                 for b in vir_b:
                     out.append(((a, b), (j, i)))
     return out
+
+
+def tfim_terms(n_qubits: int, J: float = 0.25, h: float = 1.0):
+    """Open transverse-field Ising chain H = J sum Z_i Z_{i+1} + h sum X_i (Eq. 40: J = 1/4, h = 1) as
+    (x masks, z masks, coefficients) of its 2 N - 1 Pauli strings.  Index bookkeeping only."""
+    x, z, c = [], [], []
+    for i in range(n_qubits - 1):
+        x.append(0), z.append((1 << i) | (1 << (i + 1))), c.append(J)
+    for i in range(n_qubits):
+        x.append(1 << i), z.append(0), c.append(h)
+    return np.array(x, np.uint64), np.array(z, np.uint64), np.array(c, np.complex128)
