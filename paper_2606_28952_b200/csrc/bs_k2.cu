@@ -113,6 +113,101 @@ k_aa(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i
     }
 }
 
+// Tensor-instruction form (mma.sync.m8n8k4.f64, SASS DMMA; same FP64 peak as DFMA, see profiles/r02_fp64_peak.md): a warp
+// owns 32 columns (4 row tiles of 8) x 8 NT targets.  A[column][u] = psi[source member u][column] (re and im as separate
+// tiles), B[u][target] = the coupling tile, four source members per step.  One B fragment load feeds 8 columns: the
+// warp-uniform coupling loads of the DFMA form (65 % of the shared-memory pipe, profiles/r02_q32_k_aa_full.md) shrink 12x.
+__host__ __device__ constexpr int k2_gs(int NT) { return 8 * NT + 4; }   // row stride of the coupling tile: conflict-free fragments
+
+template <int NT>
+__global__ void __launch_bounds__(kAaThreads, 2)
+k_aa_mma(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i64 L, i64 c0, i64 W, i64 row_lo,
+         i64 row_hi) {
+    extern __shared__ __align__(16) unsigned char smem_k2[];
+    constexpr int RT = 8 * NT, GS = k2_gs(NT);
+    const int P = K.P, f = blockIdx.y, t0 = blockIdx.x * RT, nt = min(RT, P - t0), tid = threadIdx.x;
+    double* sC = reinterpret_cast<double*>(smem_k2);                          // [P + 4][GS] coupling tile, source-major
+    u32* srow = reinterpret_cast<u32*>(smem_k2 + (size_t)(P + 4) * GS * 8);    // [P + 4] row of every source member
+    const u32* __restrict__ mrow = K.mrow + (size_t)f * P;
+    const u32* __restrict__ mpair = K.mpair + (size_t)f * P;
+    bool any = false;   // block-uniform: some target of the tile lies in the requested row range
+    for (int tt = 0; tt < nt; ++tt) {
+        const i64 r = __ldg(mrow + t0 + tt);
+        any |= r >= row_lo && r < row_hi;
+    }
+    if (!any) return;
+    const u32 k2 = __ldg(K.fk2 + f);
+    for (int idx = tid; idx < (P + 4) * GS; idx += kAaThreads) {
+        const int u = idx / GS, tt = idx - u * GS;
+        double v = 0.0;
+        if (u < P && tt < nt) {
+            const u32 pt = __ldg(mpair + t0 + tt), pu = __ldg(mpair + u);
+            if (!(pt & pu)) {   // disjoint pairs: a double excitation; its group by the rank of the 4-bit mask
+                const u32 g = rank4(pt | pu), t = k2 | pt;
+                const u32 s1 = __ldg(K.goff + g + 1);
+                for (u32 s = __ldg(K.goff + g); s < s1; ++s)
+                    v += flip(__ldg(K.gw + s), (u32)__popc(__ldg(K.gza + s) & t) & 1u);
+            }
+        }
+        sC[idx] = v;
+    }
+    for (int u = tid; u < P + 4; u += kAaThreads) srow[u] = u < P ? __ldg(mrow + u) : 0u;
+    __syncthreads();
+    const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, tq = lane & 3;
+    for (i64 cb = c0 + warp * 32; cb < c0 + W; cb += kAaThreads) {
+        double cr[4][NT][2], ci[4][NT][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NT; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        bool okc[4];
+        const double2* pc[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const i64 c = cb + 8 * i + g;
+            okc[i] = c < c0 + W;
+            pc[i] = psi + (okc[i] ? c : c0);
+        }
+        double2 a[4], an[4];   // this step's amplitudes, the next step's in flight
+#pragma unroll
+        for (int i = 0; i < 4; ++i) a[i] = __ldg(pc[i] + (i64)srow[tq] * L);
+        for (int u = 0; u < P; u += 4) {
+            if (u + 4 < P) {
+                const i64 ro = (i64)srow[u + 4 + tq] * L;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) an[i] = __ldg(pc[i] + ro);
+            }
+            double bf[NT];
+#pragma unroll
+            for (int j = 0; j < NT; ++j) bf[j] = sC[(u + tq) * GS + 8 * j + g];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const double are = okc[i] ? a[i].x : 0.0, aim = okc[i] ? a[i].y : 0.0;
+#pragma unroll
+                for (int j = 0; j < NT; ++j) {
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                 : "+d"(cr[i][j][0]), "+d"(cr[i][j][1]) : "d"(are), "d"(bf[j]));
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                 : "+d"(ci[i][j][0]), "+d"(ci[i][j][1]) : "d"(aim), "d"(bf[j]));
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = an[i];
+        }
+        // C fragment: row g of tile i (column cb + 8 i + g), targets 8 j + 2 tq + {0, 1}
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NT; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int tt = 8 * j + 2 * tq + e;
+                    if (okc[i] && tt < nt)
+                        S2[((i64)f * P + t0 + tt) * W + (cb + 8 * i + g - c0)] = make_double2(cr[i][j][e], ci[i][j][e]);
+                }
+    }
+}
+
 // acc[r][c] += sum_j S2[tf[r][j]][c - c0], j in fixed order
 __global__ void __launch_bounds__(256)
 k_aa_acc(const u32* __restrict__ tf, int NP2, const double2* __restrict__ S2, double2* __restrict__ acc, i64 L, i64 W,
@@ -144,8 +239,19 @@ cudaError_t kaa_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W,
     return cudaGetLastError();
 }
 
+template <int NT>
+cudaError_t kaa_mma_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi,
+                           cudaStream_t st, bool set_attr) {
+    if (set_attr) return cudaFuncSetAttribute(k_aa_mma<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    dim3 grid((unsigned)K->n_tiles, (unsigned)K->F);
+    k_aa_mma<NT><<<grid, kAaThreads, K->smem, st>>>(K->dev, psi, K->d_S2.p, L, c0, W, row_lo, row_hi);
+    return cudaGetLastError();
+}
+
 cudaError_t kaa_dispatch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi,
                          cudaStream_t st, bool set_attr) {
+    if (K->mma) return K->rt == 8 ? kaa_mma_launch<1>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr)
+                                  : kaa_mma_launch<2>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
     switch (K->rt) {
         case 4: return kaa_launch<4>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
         case 8: return kaa_launch<8>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
@@ -241,12 +347,17 @@ int bs_k2_build(std::vector<HostGroup>& groups, const std::vector<u64>& row_stri
     K->NP2 = NP2;
     K->rows = rows;
     K->n_groups = n_q;
-    // 12 targets per tile: 2 x 12 DFMA per 16-byte load still hides the load behind arithmetic, and at ~100 registers two
-    // blocks (16 warps) fit an SM; 28-target tiles (1 block, 8 warps) were 3 - 6 % slower on configs 2, 4 and 5
-    K->rt = std::min(12, (P + 3) / 4 * 4);
-    if (const char* e = getenv("BS_K2_RT")) K->rt = std::min(28, std::max(4, atoi(e) / 4 * 4));   // test hook: tile height
+    // Tensor-instruction form (default; BS_K2_MMA=0: DFMA form): tiles of 16 targets (8 when the family has <= 8 members).
+    // DFMA form: 12 targets per tile -- 2 x 12 DFMA per 16-byte load still hides the load behind arithmetic and two blocks
+    // (16 warps) fit an SM; 28-target tiles (1 block, 8 warps) were 3 - 6 % slower on configs 2, 4 and 5.
+    K->mma = getenv("BS_K2_MMA") ? atoi(getenv("BS_K2_MMA")) != 0 : true;
+    if (K->mma) K->rt = P <= 8 ? 8 : 16;
+    else {
+        K->rt = std::min(12, (P + 3) / 4 * 4);
+        if (const char* e = getenv("BS_K2_RT")) K->rt = std::min(28, std::max(4, atoi(e) / 4 * 4));   // test hook: tile height
+    }
     K->n_tiles = (P + K->rt - 1) / K->rt;
-    K->smem = (size_t)(P + 4) * K->rt * 8 + (size_t)(P + 4) * 4;
+    K->smem = (size_t)(P + 4) * (K->mma ? k2_gs(K->rt / 8) : K->rt) * 8 + (size_t)(P + 4) * 4;
     if (K->smem > 200 * 1024 || (i64)F * P >= (i64(1) << 31) || F > 65535) {
         delete K;
         return BS_OK;

@@ -31,6 +31,7 @@ struct bs_k2 {
     int n = 0, N = 0, P = 0, F = 0, NP2 = 0, rt = 0, n_tiles = 0;
     i64 rows = 0, slab_cols = 0;
     size_t smem = 0;
+    bool mma = true;        // contraction on the FP64 tensor instruction (k_aa_mma), else DFMA (k_aa)
     i64 n_groups = 0;
     std::vector<u32> h_x;   // row-spin X masks of the groups taken (bs_plan_groups)
     DevBuf<u32> d_mrow, d_mpair, d_fk2, d_goff, d_gza, d_tf;

@@ -106,7 +106,7 @@ print('PATH OK')
     ({}, "rows_v2"),
     ({"BS_NO_LIGHT": "1", "BS_NO_KRES": "1", "BS_NO_K2": "1", "BS_NO_CDIAG": "1"}, "rows_v2"),   # column-list pass and row axpys only
     ({"BS_K2_SLAB_MB": "1", "BS_K2_MIN": "1", "BS_NO_HOPSPLIT": "1"}, "kres{"),              # several column slabs of the K2 scratch
-    ({"BS_KRES_KC": "64", "BS_KRES_SLAB_MB": "2"}, "kres{"),          # more K chunks, several scratch slabs
+    ({"BS_KRES_KC": "64", "BS_KRES_SLAB_MB": "2", "BS_K2_MMA": "0"}, "kres{"),   # more K chunks, several scratch slabs, DFMA k_aa
     ({"BS_KRES_KC": "32", "BS_KRES_MIN": "1", "BS_KRES_MMA": "0"}, "kres{"),   # DFMA form of the K-resolved contraction
     ({"BS_LIGHT_COMPACT": "1", "BS_LIGHT_ORDER": "0", "BS_LIGHT_SIGN": "1"}, "rows_v2"),   # light kernel: compacted list, one phase order, signed entries
     ({"BS_LIGHT_ORDER": "1", "BS_LIGHT_THREADS": "1024"}, "rows_v2"),
