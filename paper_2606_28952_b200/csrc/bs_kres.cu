@@ -212,12 +212,19 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
 #pragma unroll
         for (int i2 = 0; i2 < RTW; ++i2) sigk[i2] = __ldg(Kd.sigma + (size_t)chunk * KC + kw + 8 * i2);
         const int n_act = __popc(act_all);
+        // this lane's orbital of every step (the (4 step + tq)-th active one), 6 bits each, 63 = none: found once per
+        // block instead of at every step of every entry (__fns is a loop)
+        u64 my_orb = 0;
+        for (int st_ = 0; st_ < 8; ++st_) {
+            const u32 s_ = 4 * st_ + tq < (u32)n_act ? __fns(act_all, 0, 4 * st_ + tq + 1) : 63u;
+            my_orb |= (u64)(s_ & 63u) << (6 * st_);
+        }
         for (int i = 0; i < n_ent; ++i) {
             mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
             const double* __restrict__ G = sG + (i & 1) * GN;
             const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
             for (int ks = 0; ks < n_act; ks += 4) {
-                const u32 s = __fns(act_all, 0, ks + tq + 1);   // this lane's orbital of the step (0xFFFFFFFF: none left)
+                const u32 s = (u32)(my_orb >> (6 * (ks >> 2))) & 63u;   // this lane's orbital of the step (63: none left)
                 const bool valid = s < 32u;
                 const u32 sc = valid ? s : 0u;
                 double are[RTW], aim[RTW], bf[NT];
