@@ -448,6 +448,26 @@ def test_p11_taylor_vs_dense_expm_and_reversibility():
     assert np.linalg.norm(psi - psi0) < 1e-12
 
 
+def test_p11_taylor_full_space_tfim_vs_dense_expm():
+    """The propagator on a number-non-conserving operator in the full 2^N space: the open TFIM chain of PAPER.md:469-473
+    (Eq. 40, J = 1/4, h = 1, dt = 0.05) from |0...0> against scipy's expm of the Kronecker-product matrix."""
+    N = 8
+    x, z, c = S.tfim_terms(N)
+    Hm = R.pauli_sum_matrix([int(v) for v in x], [int(v) for v in z], list(c), N).toarray()
+    assert np.abs(Hm - Hm.conj().T).max() == 0
+    op, sec = O.PauliOp(x, z, c), O.Sector(N)
+    psi = np.zeros(1 << N, np.complex128)
+    psi[0] = 1.0
+    e0 = O.energy(sec, op, psi).real
+    assert abs(e0 - 0.25 * (N - 1)) < 1e-14                  # every Z_i Z_{i+1} = +1 on |0...0>, <X_i> = 0
+    for _ in range(8):
+        sec.taylor_step(op, psi, 0.05, 12, e0)
+    v0 = np.zeros(1 << N, np.complex128)
+    v0[0] = 1.0
+    assert np.linalg.norm(psi - scipy.linalg.expm(-1j * Hm * 0.4) @ v0) < 1e-12
+    assert abs(np.linalg.norm(psi) - 1) < 1e-12
+
+
 # ---------------------------------------------------------------- P12 fast mode and sampled mode
 @pytest.mark.parametrize("kind", ["molecular", "hubbard", "generator", "full"])
 def test_p12_grouped_and_sampled_equal_definition(kind):
