@@ -82,10 +82,14 @@ def random_state(dim: int, seed: int) -> np.ndarray:
     psi = np.empty(dim, dtype=np.complex128)
     v = psi.view(np.float64)
     chunk = 1 << 24
+    parts = []
     for i in range(0, 2 * dim, chunk):
         j = min(2 * dim, i + chunk)
         v[i:j] = rng.standard_normal(j - i)
-    nrm = math.sqrt(float(np.dot(v, v)))
+        parts.append(float(np.sum(np.square(v[i:j]))))
+    # the squared norm by numpy's own (single-threaded, pairwise) sums per chunk: np.dot is a threaded BLAS reduction
+    # whose rounding, and with it the last bit of EVERY amplitude, changed with the host's thread count
+    nrm = math.sqrt(math.fsum(parts))
     v /= nrm
     return psi
 
