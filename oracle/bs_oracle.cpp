@@ -545,6 +545,10 @@ void orc_rot_fermionic(void* s, const int* cre, int n_cre, const int* ann, int n
     Sector* S = (Sector*)s;
     cd* psi = (cd*)psi_reim;
     double c = std::cos(theta), sn = std::sin(theta);
+    // The iterations are independent: iteration i touches psi[i] and psi[it] only when T|i> != 0, then T|it> = 0
+    // (T^2 = 0 on a configuration it has just excited), so iteration `it` touches nothing, and T is injective on its
+    // support, so no other source reaches `it`.  Same arithmetic per pair as the serial loop, in any order.
+#pragma omp parallel for schedule(static)
     for (i64 i = 0; i < S->D; ++i) {
         u64 cfg = S->config(i), t;
         int sg;
