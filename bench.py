@@ -12,6 +12,8 @@ exp(-i H dt) (a7: 12 fused apply+axpby launches of the a4 kernel, terms accumula
 reported as setup_ms; a6 (rotations) is timed in the q24 entry of `per_config`.
 value = H applications per second over all ranks (each rank propagates its own state: weak scaling,
 no data-path collective).  See DESIGN.md "Measurement" for the byte counts behind `roofline`.
+With --workload q12 | q24 | q32 | q56 (molecular configs) a step is one bs_apply + one bs_expect = 2 H applications
+ and `roofline` is reported against the FP64 pipe, which is what binds them.
 """
 from __future__ import annotations
 
@@ -102,6 +104,13 @@ def build_operator(name: str, bs):
     return bs.bs_jw_molecular(h, g), 8 * n * n + 64 * n ** 4
 
 
+def nnz_per_row(cfg) -> int:
+    """Non-zeros per row of a molecular H in the sector for generic integrals (closed form)."""
+    from math import comb
+    oa, va, ob, vb = cfg.n_alpha, cfg.n_orb - cfg.n_alpha, cfg.n_beta, cfg.n_orb - cfg.n_beta
+    return 1 + oa * va + ob * vb + comb(oa, 2) * comb(va, 2) + comb(ob, 2) * comb(vb, 2) + oa * va * ob * vb
+
+
 def table_bytes(op) -> int:
     """Group-table bytes of the a2 layout: xg u64[G] + offs i64[G+1] + z u64[M] + w c128[M]."""
     return 8 * op.n_groups + 8 * (op.n_groups + 1) + 24 * op.n_terms
@@ -148,10 +157,7 @@ def per_config_entry(name: str, bs, torch, peak_gbs: float, flush_buf, with_cpu:
            "apply_ms": apply_ms, "applies_per_s": 1e3 / apply_ms, "reps": max(reps, 1),
            "l2_flush_between_reps": bool(flush)}
     if cfg.kind == "molecular":       # non-zeros per row of H in the sector for generic integrals
-        from math import comb
-        oa, va, ob, vb = cfg.n_alpha, cfg.n_orb - cfg.n_alpha, cfg.n_beta, cfg.n_orb - cfg.n_beta
-        nnz_row = 1 + oa * va + ob * vb + comb(oa, 2) * comb(va, 2) + comb(ob, 2) * comb(vb, 2) + oa * va * ob * vb
-        ent["nonzeros_per_s"] = nnz_row * cfg.dim / (apply_ms * 1e-3)
+        ent["nonzeros_per_s"] = nnz_per_row(cfg) * cfg.dim / (apply_ms * 1e-3)
         ent["gather_gbs"] = 16 * ent["nonzeros_per_s"] / 1e9      # 16-byte amplitude gathers through L2 / shared memory
         # Resources that bind these configs: one 16-byte amplitude per non-zero through the
         # shared-memory / L1 path (128 B/clk/SM) and 2 DFMA per non-zero (real weight x complex amplitude) on the FP64
@@ -314,8 +320,20 @@ def run_ours(args):
     tb = table_bytes(op)
     ev = lambda: torch.cuda.Event(enable_timing=True)    # noqa: E731
 
+    # What a step is ("Work timed"): the lattice model is propagated (configs[2]: Taylor-12
+    # steps); the molecular configs time one H application + one expectation (their order-12 series at dt = 0.05 does
+    # not converge: the spectrum of the synthetic molecular H is two orders of magnitude wider than the chain's).
+    taylor = cfg.kind == "hubbard"
+    outs_dev = [work[:D], work[D:]]      # molecular steps: H psi lands here (bs_apply uses no work space)
+
+    def main_op(vec, k=0):
+        if taylor:
+            bs.bs_taylor_step(op, sec, vec, work, DT, TAYLOR_ORDER, e_shift)
+        else:
+            bs.bs_apply(op, sec, vec, outs_dev[k])
+
     def step():
-        bs.bs_taylor_step(op, sec, psi, work, DT, TAYLOR_ORDER, e_shift)
+        main_op(psi)
         return bs.bs_expect(op, sec, psi)
 
     def barrier():
@@ -338,7 +356,7 @@ def run_ours(args):
     marks[0].record()
     energy = None
     for i in range(args.steps):
-        bs.bs_taylor_step(op, sec, psi, work, DT, TAYLOR_ORDER, e_shift)
+        main_op(psi)
         marks[2 * i + 1].record()
         energy = bs.bs_expect(op, sec, psi)
         marks[2 * i + 2].record()
@@ -379,12 +397,14 @@ def run_ours(args):
         if i + 1 < e2e_steps:
             h2d(i + 1)
         s_main.wait_event(ev_in[i])
-        bs.bs_taylor_step(op, sec, bufs[i % 2], work, DT, TAYLOR_ORDER, e_shift)
+        main_op(bufs[i % 2], i % 2)
         bs.bs_expect(op, sec, bufs[i % 2])                 # 16-byte result, synchronises the compute stream
         ev_c[i].record(s_main)
         with torch.cuda.stream(s_out):
             s_out.wait_event(ev_c[i])
-            outs_h[i % 2].copy_(bufs[i % 2], non_blocking=True)
+            # the step's result: the propagated state, or H psi.  Output half i % 2 is next written by step i + 2,
+            # which waits for ev_out[i] through its input buffer (h2d), so this copy may overlap step i + 1
+            outs_h[i % 2].copy_(bufs[i % 2] if taylor else outs_dev[i % 2], non_blocking=True)
             ev_out[i].record(s_out)
     s_main.wait_event(ev_out[e2e_steps - 1])
     if e2e_steps > 1:
@@ -398,7 +418,7 @@ def run_ours(args):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms, e2e_ms, taylor_ms, expect_ms = t.tolist()
-    applies_per_step = TAYLOR_ORDER + 1
+    applies_per_step = TAYLOR_ORDER + 1 if taylor else 2
     if rank == 0:
         value = world * applies_per_step * args.steps / (total_ms * 1e-3)
         # dominant kernel: the apply kernel of the Taylor launches. Algorithmic bytes per Taylor step (bs_taylor_step
@@ -409,6 +429,30 @@ def run_ours(args):
         bytes_taylor = sum(per_launch) * D + TAYLOR_ORDER * tb
         launch_ms = taylor_ms / (args.steps * TAYLOR_ORDER)
         achieved = bytes_taylor / TAYLOR_ORDER / launch_ms / 1e6
+        plan = bs.bs_plan_describe(op, sec)
+        if taylor:
+            step_txt = (f"1 Taylor-{TAYLOR_ORDER} step (dt={DT}, shifted) + 1 bs_expect = {applies_per_step} H applies")
+            roofline = {"bound": "hbm", "kernel": ("k_light<0>" if "+light" in plan else "k_rows<MODE_FINAL>")
+                        + " (the 12 apply+axpby launches of bs_taylor_step)",
+                        "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
+                        "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
+                        "launch_ms": launch_ms, "traffic": (TRAFFIC_NCU.get(name) or {}).get("bytes_per_launch"),
+                        "traffic_source": (TRAFFIC_NCU.get(name) or {}).get("profile")}
+        else:
+            # Molecular configs: thousands of non-zeros per target, the compulsory-bytes roofline is out of reach of any
+            # exact method; what binds is the FP64 pipe (k_ab / k_aa on the FP64 tensor
+            # instruction).  2 FMA = 4 flops per non-zero (real weight x complex amplitude) over the plain bs_apply;
+            # peak = 64 FMA/clk/SM measured (profiles/r02_fp64_peak.md) x 148 SMs x 1.965 GHz x 2 flops.
+            step_txt = "1 bs_apply + 1 bs_expect = 2 H applies"
+            apply_ms = taylor_ms / args.steps
+            flops = 4.0 * nnz_per_row(cfg) * D
+            roofline = {"bound": "alu", "kernel": "k_ab + k_aa_mma (FP64 tensor instruction) of one bs_apply",
+                        "achieved": flops / (apply_ms * 1e-3) / 1e12, "peak": 2 * DFMA_PEAK / 1e12, "unit": "TFLOP/s",
+                        "frac": flops / (apply_ms * 1e-3) / (2 * DFMA_PEAK),
+                        "peak_source": "derived: measured 64 FP64 FMA/clk/SM (profiles/r02_fp64_peak.md) x 148 SMs x 1.965 GHz",
+                        "flops_per_launch": flops, "launch_ms": apply_ms, "useful_flops_only": True,
+                        "traffic": (TRAFFIC_NCU.get(name) or {}).get("bytes_per_launch"),
+                        "traffic_source": (TRAFFIC_NCU.get(name) or {}).get("profile")}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -416,23 +460,19 @@ def run_ours(args):
             "config": {"workload": f"{name}: BASELINE.json configs[{si.CONFIG_ORDER.index(name)}]",
                        "n_qubits": cfg.n_qubits, "sector": [cfg.n_orb, cfg.n_alpha, cfg.n_beta], "dim": D,
                        "groups": op.n_groups, "strings": op.n_terms,
-                       "step": f"1 Taylor-{TAYLOR_ORDER} step (dt={DT}, shifted) + 1 bs_expect = "
-                               f"{applies_per_step} H applies",
-                       "l2": "3 vectors x 188.5 MB > 126 MB L2, no flush needed",
+                       "step": step_txt,
+                       "l2": (f"vectors of {16 * D / 1e6:.1f} MB each exceed the 126 MB L2, no flush needed" if 16 * D > 126e6
+                              else f"vectors of {16 * D / 1e6:.1f} MB fit the 126 MB L2 and are NOT flushed between steps "
+                                   "(the per_config sweep flushes)"),
                        "parallelism": f"{world} independent state vector(s), one per GPU",
-                       "plan": bs.bs_plan_describe(op, sec)},
-            "setup_ms": setup_ms, "taylor_ms_per_step": taylor_ms / args.steps,
+                       "plan": plan},
+            "setup_ms": setup_ms, ("taylor_ms_per_step" if taylor else "apply_ms_per_step"): taylor_ms / args.steps,
             "expect_ms_per_call": expect_ms / args.steps, "energy": energy.real, "norm_drift": norm_drift,
             "gpu_launches": int(launches), "clocks": clocks,
             "e2e": {"value": world * applies_per_step * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 16 * D, "d2h_bytes_per_step": 16 * D + 16, "steps": e2e_steps,
                     "pipeline": "H2D of step i+1 and D2H of step i-1 overlap step i (2 device buffers, 3 streams)"},
-            "roofline": {"bound": "hbm", "kernel": ("k_light<0>" if "+light" in bs.bs_plan_describe(op, sec) else "k_rows<MODE_FINAL>")
-                         + " (the 12 apply+axpby launches of bs_taylor_step)",
-                         "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
-                         "peak_source": peak_src, "bytes_per_launch": bytes_taylor / TAYLOR_ORDER,
-                         "launch_ms": launch_ms, "traffic": (TRAFFIC_NCU.get(name) or {}).get("bytes_per_launch"),
-                         "traffic_source": (TRAFFIC_NCU.get(name) or {}).get("profile")},
+            "roofline": roofline,
         }
         want = [] if args.per_config == "none" else args.per_config.split(",")
         if want and world == 1:

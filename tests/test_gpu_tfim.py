@@ -99,3 +99,34 @@ def test_diagonal_generator_in_a_sector():
         state = acc
     assert rel_l2(d.cpu().numpy(), state) <= 1e-12
     assert abs(np.linalg.norm(d.cpu().numpy()) - 1.0) <= 1e-12
+
+
+@pytest.mark.parametrize("N", [10, 14])
+def test_tfim_taylor_propagation_in_the_full_space(N):
+    """a7 on a number-non-conserving operator: shifted order-12 Taylor steps (Eq. 6-7; dt = 0.05 as in
+    PAPER.md:473) of the TFIM chain in the full 2^N space against the oracle's own propagator, started from the
+    paper's initial state |0...0>; norm and energy conserved."""
+    import torch
+    from oracle import oracle as orc
+    from paper_2606_28952_b200 import bs
+    x, z, c = si.tfim_terms(N)
+    op = bs.bs_group_xmask(x, z, c, N, 0.0)
+    ref = orc.PauliOp(x, z, c)
+    sec, osec = bs.bs_sector_build(N), orc.Sector(N)
+    psi = np.zeros(1 << N, np.complex128)
+    psi[0] = 1.0
+    d = torch.from_numpy(psi.copy()).cuda()
+    work = torch.empty(2 << N, dtype=torch.complex128, device="cuda")
+    e0 = bs.bs_expect(op, sec, d).real
+    assert abs(e0 - 0.25 * (N - 1)) <= 1e-12                            # <0|H|0> = J (N - 1): every Z_i Z_{i+1} = +1
+    for _ in range(6):
+        bs.bs_taylor_step(op, sec, d, work, 0.05, 12, e0)
+        osec.taylor_step(ref, psi, 0.05, 12, e0)
+    got = d.cpu().numpy()
+    assert rel_l2(got, psi) <= 1e-12
+    assert abs(np.linalg.norm(got) - 1.0) <= 1e-12
+    assert abs(bs.bs_expect(op, sec, d).real - e0) <= 1e-10
+    # total transverse magnetisation sum_i <X_i> (Figure 5's observable) through the same fused expectation
+    mx = bs.bs_group_xmask(x[N - 1:], z[N - 1:], np.ones(N, np.complex128), N, 0.0)
+    want = orc.vdot(psi, osec.apply(orc.PauliOp(x[N - 1:], z[N - 1:], np.ones(N, np.complex128)), psi))
+    assert abs(bs.bs_expect(mx, sec, d) - want) <= 1e-10

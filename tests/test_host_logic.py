@@ -139,3 +139,25 @@ def test_sharded_apply_gloo(world, tmp_path):
     env = dict(os.environ, OMP_NUM_THREADS="1")
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=env)
     assert r.returncode == 0 and r.stdout.count("RANK_OK") == world, r.stdout[-2000:] + r.stderr[-3000:]
+
+
+def test_bench_nonzero_count_matches_the_survey_table_and_the_oracle():
+    """bench.py's flop count for the molecular configs (4 flops per non-zero) rests on the closed form for the
+    non-zeros per row of H in a sector: 118 / 1,819 / 5,793 / 12,721 at configs 1, 2, 4, 5.
+    At config 1 it is also counted by brute force from the oracle: the sector matrix of H, column by column."""
+    import importlib.util
+    from oracle import oracle as orc
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    want = {"q12": 118, "q24": 1819, "q32": 5793, "q56": 12721}
+    for name, nnz in want.items():
+        assert bench.nnz_per_row(si.CONFIGS[name]) == nnz
+    cfg = si.CONFIGS["q12"]
+    op = orc.molecular_h(*si.integrals(cfg.n_orb, cfg.seed_ints))
+    sec = orc.Sector(cfg.n_orb, cfg.n_alpha, cfg.n_beta)
+    eye = np.eye(sec.dim, dtype=np.complex128)
+    hm = np.column_stack([sec.apply(op, eye[:, k].copy()) for k in range(sec.dim)])
+    per_row = (np.abs(hm) > 1e-13).sum(axis=1)
+    assert per_row.max() == 118 and int(per_row.sum()) == 47200      # generic integrals: every allowed element is non-zero
