@@ -59,11 +59,13 @@ def _golden_module():
 
 
 def _golden(name):
-    """Full-size goldens written by tests/golden/make_fullsize_golden.py from oracle/ only (see its docstring)."""
+    """Full-size goldens written from oracle/ only by tests/golden/make_fullsize_golden.py (H psi) and
+    tests/golden/make_rotation_golden.py (the *_rot files); see their docstrings."""
     import os
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"fullsize_{name}.npz")
     if not os.path.exists(path):
-        pytest.skip(f"{path} not generated yet (hours of oracle time): run tests/golden/make_fullsize_golden.py {name}")
+        script = "make_rotation_golden.py" if name.endswith("_rot") else f"make_fullsize_golden.py {name}"
+        pytest.skip(f"{path} not generated yet (minutes to hours of oracle time): run tests/golden/{script}")
     return np.load(path)
 
 
@@ -127,7 +129,8 @@ def test_q32_uccsd_rotations(bs):
     fits shared memory, so runs of generators go through the pair-list kernel, one launch per generator.
     (i) 16 orbitals, (2, 8) electrons (D_beta = 12,870 as in configs[3], D = 1.5e6 so that the single-threaded oracle
     finishes): 600 of its 2,759 UCCSD generators, in list order, on a random state, full-vector comparison with the
-    oracle's fermionic Givens rotations.  (ii) configs[3] itself, all 5,792 generators (43,264 Pauli strings): norm."""
+    oracle's fermionic Givens rotations.  (ii) configs[3] itself, all 5,792 generators (43,264 Pauli strings): norm, and
+    (iii) the rotated vector against the oracle's result for the whole list (stored golden)."""
     import torch
     from oracle import oracle as orc
     from paper_2606_28952_b200 import jw_terms as jw
@@ -158,3 +161,16 @@ def test_q32_uccsd_rotations(bs):
     d = torch.from_numpy(si.random_state(cfg.dim, cfg.seed_psi)).cuda()
     bs.bs_apply_pauli_rotations(gens, sec, si.thetas(len(ex), 3004), d)
     assert abs(np.sqrt(bs.bs_vdot(sec, d, d).real) - 1.0) <= 1e-10
+    # (iii) the rotated vector against the oracle's fermionic Givens rotations over the WHOLE list
+    # (tests/golden/make_rotation_golden.py, oracle/ only): every row and column through its complex sum, every row
+    # through its norm, 65,536 sampled amplitudes and four complete rows element by element
+    z = _golden("q32_rot")
+    assert int(z["n_generators"]) == len(ex) and int(z["theta_seed"]) == 3004
+    d2 = d.view(cfg.dim_alpha, cfg.dim_beta)
+    assert rel_l2(d2.sum(dim=1).cpu().numpy(), z["row_sum"]) <= 1e-11
+    assert rel_l2(d2.sum(dim=0).cpu().numpy(), z["col_sum"]) <= 1e-11
+    assert rel_l2((d2.real ** 2 + d2.imag ** 2).sum(dim=1).cpu().numpy(), z["row_n2"]) <= 1e-12
+    idx = torch.from_numpy(z["sample_idx"]).cuda()
+    assert rel_l2(d[idx].cpu().numpy(), z["sample_val"]) <= 1e-12
+    rows = torch.from_numpy(z["rows"]).cuda()
+    assert rel_l2(d2[rows].cpu().numpy(), z["row_val"]) <= 1e-12
