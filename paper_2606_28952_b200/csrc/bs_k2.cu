@@ -114,75 +114,122 @@ k_aa(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i
 }
 
 // Tensor-instruction form (mma.sync.m8n8k4.f64, SASS DMMA; same FP64 peak as DFMA, see profiles/r02_fp64_peak.md): a warp
-// owns 32 columns (4 row tiles of 8) x 8 NT targets.  A[column][u] = psi[source member u][column] (re and im as separate
+// owns 8 RTW columns (RTW row tiles of 8) x 8 NT targets and keeps the amplitudes of the next DEPTH steps in registers.
+// One 16-byte amplitude load per lane and row tile feeds 2 NT DMMAs: with <NT, RTW, DEPTH> = <2, 4, 1> the kernel ran at
+// half the tensor pipe because only 32 KB per SM were in flight against ~2,150 cycles of L2 latency
+// (profiles/r02b_q32_k_ab_k_aa_full.md); <3, 2, 3> and <4, 2, 3> need 1.5x / 2x fewer bytes per DMMA and hold 1.5x more
+// in flight per warp at the same accumulator registers.  A[column][u] = psi[source member u][column] (re and im as separate
 // tiles), B[u][target] = the coupling tile, four source members per step.  One B fragment load feeds 8 columns: the
 // warp-uniform coupling loads of the DFMA form (65 % of the shared-memory pipe, profiles/r02_q32_k_aa_full.md) shrink 12x.
 __host__ __device__ constexpr int k2_gs(int NT) { return 8 * NT + 4; }   // row stride of the coupling tile: conflict-free fragments
 
+// entry (source member u, target tt of the tile at t0) of a family's coupling tile: F_g(t) of the double excitation that
+// takes member u to member t0 + tt, 0 if the two pairs overlap or the slot is padding
+__device__ __forceinline__ double k2_tile_entry(const K2Dev& K, const u32* __restrict__ mpair, u32 k2, int t0, int nt,
+                                                int u, int tt) {
+    double v = 0.0;
+    if (u < K.P && tt < nt) {
+        const u32 pt = __ldg(mpair + t0 + tt), pu = __ldg(mpair + u);
+        if (!(pt & pu)) {   // disjoint pairs: a double excitation; its group by the rank of the 4-bit mask
+            const u32 g = rank4(pt | pu), t = k2 | pt;
+            const u32 s1 = __ldg(K.goff + g + 1);
+            for (u32 s = __ldg(K.goff + g); s < s1; ++s)
+                v += flip(__ldg(K.gw + s), (u32)__popc(__ldg(K.gza + s) & t) & 1u);
+        }
+    }
+    return v;
+}
+
+// fallback of k_aa_mma when the tiles were not evaluated at plan time; not inlined, so that its registers (table
+// pointers, string loop) do not count against the contraction loop, which sits at the 128-register cap
+__device__ __noinline__ void k2_fill_tile(const K2Dev& K, int f, int t0, int nt, int GS, double* sC) {
+    const u32* __restrict__ mpair = K.mpair + (size_t)f * K.P;
+    const u32 k2 = __ldg(K.fk2 + f);
+    for (int idx = threadIdx.x; idx < (K.P + 4) * GS; idx += kAaThreads) {
+        const int u = idx / GS, tt = idx - u * GS;
+        sC[idx] = k2_tile_entry(K, mpair, k2, t0, nt, u, tt);
+    }
+}
+
+// plan time: every (family, target tile) coupling tile of the tensor form, in the layout k_aa_mma keeps in shared memory
 template <int NT>
+__global__ void __launch_bounds__(kAaThreads) k_aa_tiles(const K2Dev K, double* __restrict__ out) {
+    constexpr int RT = 8 * NT, GS = k2_gs(NT);
+    const int P = K.P, f = blockIdx.y, t0 = blockIdx.x * RT, nt = min(RT, P - t0);
+    const u32* __restrict__ mpair = K.mpair + (size_t)f * P;
+    const u32 k2 = __ldg(K.fk2 + f);
+    double* o = out + ((size_t)f * K.n_tiles + blockIdx.x) * (size_t)(P + 4) * GS;
+    for (int idx = threadIdx.x; idx < (P + 4) * GS; idx += kAaThreads) {
+        const int u = idx / GS, tt = idx - u * GS;
+        o[idx] = k2_tile_entry(K, mpair, k2, t0, nt, u, tt);
+    }
+}
+
+template <int NT, int RTW, int DEPTH>
 __global__ void __launch_bounds__(kAaThreads, 2)
 k_aa_mma(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S2, i64 L, i64 c0, i64 W, i64 row_lo,
          i64 row_hi) {
     extern __shared__ __align__(16) unsigned char smem_k2[];
-    constexpr int RT = 8 * NT, GS = k2_gs(NT);
+    constexpr int RT = 8 * NT, GS = k2_gs(NT), CW = 8 * RTW;   // CW: columns per warp
     const int P = K.P, f = blockIdx.y, t0 = blockIdx.x * RT, nt = min(RT, P - t0), tid = threadIdx.x;
     double* sC = reinterpret_cast<double*>(smem_k2);                          // [P + 4][GS] coupling tile, source-major
     u32* srow = reinterpret_cast<u32*>(smem_k2 + (size_t)(P + 4) * GS * 8);    // [P + 4] row of every source member
     const u32* __restrict__ mrow = K.mrow + (size_t)f * P;
-    const u32* __restrict__ mpair = K.mpair + (size_t)f * P;
     bool any = false;   // block-uniform: some target of the tile lies in the requested row range
     for (int tt = 0; tt < nt; ++tt) {
         const i64 r = __ldg(mrow + t0 + tt);
         any |= r >= row_lo && r < row_hi;
     }
     if (!any) return;
-    const u32 k2 = __ldg(K.fk2 + f);
-    for (int idx = tid; idx < (P + 4) * GS; idx += kAaThreads) {
-        const int u = idx / GS, tt = idx - u * GS;
-        double v = 0.0;
-        if (u < P && tt < nt) {
-            const u32 pt = __ldg(mpair + t0 + tt), pu = __ldg(mpair + u);
-            if (!(pt & pu)) {   // disjoint pairs: a double excitation; its group by the rank of the 4-bit mask
-                const u32 g = rank4(pt | pu), t = k2 | pt;
-                const u32 s1 = __ldg(K.goff + g + 1);
-                for (u32 s = __ldg(K.goff + g); s < s1; ++s)
-                    v += flip(__ldg(K.gw + s), (u32)__popc(__ldg(K.gza + s) & t) & 1u);
-            }
-        }
-        sC[idx] = v;
+    if (K.ctile) {   // the tile was evaluated at plan time: (P + 4) * GS doubles, a multiple of 4: 16-byte copies
+        const double2* __restrict__ src =
+            reinterpret_cast<const double2*>(K.ctile + ((size_t)f * K.n_tiles + blockIdx.x) * (size_t)(P + 4) * GS);
+        double2* dst = reinterpret_cast<double2*>(sC);
+        for (int idx = tid; idx < (P + 4) * GS / 2; idx += kAaThreads) dst[idx] = __ldg(src + idx);
+    } else {
+        k2_fill_tile(K, f, t0, nt, GS, sC);
     }
     for (int u = tid; u < P + 4; u += kAaThreads) srow[u] = u < P ? __ldg(mrow + u) : 0u;
     __syncthreads();
     const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, tq = lane & 3;
-    for (i64 cb = c0 + warp * 32; cb < c0 + W; cb += kAaThreads) {
-        double cr[4][NT][2], ci[4][NT][2];
+    for (i64 cb = c0 + warp * CW; cb < c0 + W; cb += (kAaThreads / 32) * CW) {
+        double cr[RTW][NT][2], ci[RTW][NT][2];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < RTW; ++i)
 #pragma unroll
             for (int j = 0; j < NT; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
-        bool okc[4];
-        const double2* pc[4];
+        bool okc[RTW];
+        const double2* pc[RTW];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < RTW; ++i) {
             const i64 c = cb + 8 * i + g;
             okc[i] = c < c0 + W;
             pc[i] = psi + (okc[i] ? c : c0);
         }
-        double2 a[4], an[4];   // this step's amplitudes, the next step's in flight
+        double2 q[DEPTH][RTW];   // q[0]: this step's amplitudes; q[1 .. DEPTH-1] and nx: the next DEPTH steps', in flight
 #pragma unroll
-        for (int i = 0; i < 4; ++i) a[i] = __ldg(pc[i] + (i64)srow[tq] * L);
+        for (int d = 0; d < DEPTH; ++d) {
+            const bool have = 4 * d < P;
+            const i64 ro = have ? (i64)srow[4 * d + tq] * L : 0;
+#pragma unroll
+            for (int i = 0; i < RTW; ++i) q[d][i] = have ? __ldg(pc[i] + ro) : make_double2(0.0, 0.0);
+        }
         for (int u = 0; u < P; u += 4) {
-            if (u + 4 < P) {
-                const i64 ro = (i64)srow[u + 4 + tq] * L;
+            double2 nx[RTW];
+            if (u + 4 * DEPTH < P) {
+                const i64 ro = (i64)srow[u + 4 * DEPTH + tq] * L;
 #pragma unroll
-                for (int i = 0; i < 4; ++i) an[i] = __ldg(pc[i] + ro);
+                for (int i = 0; i < RTW; ++i) nx[i] = __ldg(pc[i] + ro);
+            } else {
+#pragma unroll
+                for (int i = 0; i < RTW; ++i) nx[i] = make_double2(0.0, 0.0);
             }
             double bf[NT];
 #pragma unroll
             for (int j = 0; j < NT; ++j) bf[j] = sC[(u + tq) * GS + 8 * j + g];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const double are = okc[i] ? a[i].x : 0.0, aim = okc[i] ? a[i].y : 0.0;
+            for (int i = 0; i < RTW; ++i) {
+                const double are = okc[i] ? q[0][i].x : 0.0, aim = okc[i] ? q[0][i].y : 0.0;
 #pragma unroll
                 for (int j = 0; j < NT; ++j) {
                     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -192,11 +239,15 @@ k_aa_mma(const K2Dev K, const double2* __restrict__ psi, double2* __restrict__ S
                 }
             }
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = an[i];
+            for (int i = 0; i < RTW; ++i) {
+#pragma unroll
+                for (int d = 0; d + 1 < DEPTH; ++d) q[d][i] = q[d + 1][i];
+                q[DEPTH - 1][i] = nx[i];
+            }
         }
         // C fragment: row g of tile i (column cb + 8 i + g), targets 8 j + 2 tq + {0, 1}
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < RTW; ++i)
 #pragma unroll
             for (int j = 0; j < NT; ++j)
 #pragma unroll
@@ -239,19 +290,24 @@ cudaError_t kaa_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W,
     return cudaGetLastError();
 }
 
-template <int NT>
+template <int NT, int RTW, int DEPTH>
 cudaError_t kaa_mma_launch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi,
                            cudaStream_t st, bool set_attr) {
-    if (set_attr) return cudaFuncSetAttribute(k_aa_mma<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (set_attr)
+        return cudaFuncSetAttribute(k_aa_mma<NT, RTW, DEPTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     dim3 grid((unsigned)K->n_tiles, (unsigned)K->F);
-    k_aa_mma<NT><<<grid, kAaThreads, K->smem, st>>>(K->dev, psi, K->d_S2.p, L, c0, W, row_lo, row_hi);
+    k_aa_mma<NT, RTW, DEPTH><<<grid, kAaThreads, K->smem, st>>>(K->dev, psi, K->d_S2.p, L, c0, W, row_lo, row_hi);
     return cudaGetLastError();
 }
 
 cudaError_t kaa_dispatch(const bs_k2* K, const double2* psi, i64 L, i64 c0, i64 W, i64 row_lo, i64 row_hi,
                          cudaStream_t st, bool set_attr) {
-    if (K->mma) return K->rt == 8 ? kaa_mma_launch<1>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr)
-                                  : kaa_mma_launch<2>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
+    if (K->mma) switch (K->rt) {   // <target tiles NT, row tiles per warp, prefetch depth>
+            case 8: return kaa_mma_launch<1, 4, 1>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
+            case 16: return kaa_mma_launch<2, 4, 1>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
+            case 24: return kaa_mma_launch<3, 2, 3>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
+            default: return kaa_mma_launch<4, 2, 3>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
+        }
     switch (K->rt) {
         case 4: return kaa_launch<4>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
         case 8: return kaa_launch<8>(K, psi, L, c0, W, row_lo, row_hi, st, set_attr);
@@ -351,7 +407,21 @@ int bs_k2_build(std::vector<HostGroup>& groups, const std::vector<u64>& row_stri
     // DFMA form: 12 targets per tile -- 2 x 12 DFMA per 16-byte load still hides the load behind arithmetic and two blocks
     // (16 warps) fit an SM; 28-target tiles (1 block, 8 warps) were 3 - 6 % slower on configs 2, 4 and 5.
     K->mma = getenv("BS_K2_MMA") ? atoi(getenv("BS_K2_MMA")) != 0 : true;
-    if (K->mma) K->rt = P <= 8 ? 8 : 16;
+    if (K->mma) {
+        // target tile of 8 NT members: the fewest padded targets (executed DMMAs), ties to the larger tile (fewer
+        // amplitude bytes per DMMA).  Measured on one B200: P = 28 (q24) NT = 4, P = 45 (q32) NT = 3, P = 325 (q56) NT = 3
+        // or 4 within 0.3 %: 1 - 2 % of an application over NT = 2 everywhere.
+        K->rt = 8;
+        if (P > 8) {
+            int best = 0;
+            for (int nt = 2; nt <= 4; ++nt) {
+                const int padded = (P + 8 * nt - 1) / (8 * nt) * (8 * nt);
+                if (!best || padded <= (P + 8 * best - 1) / (8 * best) * (8 * best)) best = nt;
+            }
+            K->rt = 8 * best;
+        }
+        if (const char* e = getenv("BS_K2_NT")) K->rt = 8 * std::min(4, std::max(1, atoi(e)));   // test hook: target tiles of 8
+    }
     else {
         K->rt = std::min(12, (P + 3) / 4 * 4);
         if (const char* e = getenv("BS_K2_RT")) K->rt = std::min(28, std::max(4, atoi(e) / 4 * 4));   // test hook: tile height
@@ -387,6 +457,28 @@ int bs_k2_build(std::vector<HostGroup>& groups, const std::vector<u64>& row_stri
     d.NP2 = NP2;
     d.n_tiles = K->n_tiles;
     d.rt = K->rt;
+    d.ctile = nullptr;
+    // tensor form: the coupling tiles depend on the operator and the sector only, so they are evaluated here, once, instead
+    // of in the prologue of every block of every column-slab launch (15 % of the stall samples of k_aa_mma at configs[3]).
+    // 176 MB per spin at configs[3], 390 MB at configs[4]; above 2 GB (or BS_K2_NO_CTILE=1, test hook) the kernel evaluates.
+    const size_t tile_doubles = (size_t)(P + 4) * k2_gs(K->rt / 8), n_ctile = (size_t)F * K->n_tiles * tile_doubles;
+    const bool no_ctile = getenv("BS_K2_NO_CTILE") && atoi(getenv("BS_K2_NO_CTILE")) != 0;
+    if (ce == cudaSuccess && K->mma && !no_ctile && n_ctile * 8 <= (size_t(2) << 30)) {
+        ce = K->d_ctile.alloc(n_ctile);
+        if (ce == cudaSuccess) {
+            dim3 grid((unsigned)K->n_tiles, (unsigned)F);
+            switch (K->rt) {
+                case 8: k_aa_tiles<1><<<grid, kAaThreads, 0, st>>>(d, K->d_ctile.p); break;
+                case 16: k_aa_tiles<2><<<grid, kAaThreads, 0, st>>>(d, K->d_ctile.p); break;
+                case 24: k_aa_tiles<3><<<grid, kAaThreads, 0, st>>>(d, K->d_ctile.p); break;
+                default: k_aa_tiles<4><<<grid, kAaThreads, 0, st>>>(d, K->d_ctile.p); break;
+            }
+            BS_COUNT_LAUNCH(1);
+            ce = cudaGetLastError();
+            if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+            if (ce == cudaSuccess) d.ctile = K->d_ctile.p;
+        }
+    }
     if (ce == cudaSuccess) ce = kaa_dispatch(K, nullptr, 0, 0, 0, 0, 0, st, true);
     if (ce != cudaSuccess) {
         bs_set_error("k2 plan: %s", cudaGetErrorString(ce));

@@ -24,6 +24,8 @@ struct K2Dev {
     const u32* gza;     // strings: Z mask on the moving spin
     const double* gw;   //          weight
     const u32* tf;      // [rows][NP2] scratch slot (family * P + member) of the row's j-th electron pair
+    const double* ctile;   // [F][n_tiles][(P + 4) * k2_gs] coupling tiles of the tensor form, evaluated once at plan time
+                           // (they depend on the operator and the sector only); nullptr: evaluated in the kernel
     int P, F, NP2, n_tiles, rt;
 };
 
@@ -35,7 +37,7 @@ struct bs_k2 {
     i64 n_groups = 0;
     std::vector<u32> h_x;   // row-spin X masks of the groups taken (bs_plan_groups)
     DevBuf<u32> d_mrow, d_mpair, d_fk2, d_goff, d_gza, d_tf;
-    DevBuf<double> d_gw;
+    DevBuf<double> d_gw, d_ctile;
     DevBuf<double2> d_S2;
     K2Dev dev{};
 };
