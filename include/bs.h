@@ -39,7 +39,8 @@
  *   - up to 3 state-vector-sized scratch buffers (transposed psi, transposed result, raw H psi) when beta-only
  *     groups run on the transposed problem (every molecular Hamiltonian): 3 x 16 x dim bytes (20 GB at config 5);
  *   - the scratch of the K-resolved alpha-beta kernel: n_orb x D_K x 16 bytes per alpha row of a slab, at most 4 GiB,
- *     plus its coupling matrices (<= 2.2 GB at config 5); the scratch of the K2-resolved same-spin kernels: 2 x 4 GiB.
+ *     plus its coupling matrices (<= 2.2 GB at config 5); the scratch of the K2-resolved same-spin kernels: 2 x 4 GiB,
+ *     plus their coupling tiles evaluated at plan build (2 x 176 MB at config 4, 2 x 390 MB at config 5; none above 2 GB).
  *
  * Environment (TEST HOOKS, not API; every one is read ONCE, when a plan is built, never on a launch path):
  *   BS_KERNEL=v1|v2inrow   force the v1 sector kernel / keep beta-only groups in-row

@@ -520,7 +520,8 @@ void orc_vdot(const double* a_reim, const double* b_reim, i64 D, double* res) {
 // (spin-orbital indices, operators applied right to left)  -- Eq. 39, §2.5
 // (PAPER.md:347); SURVEY.md §8(c) item 6.  For every sector configuration s with T|s> = sg|t>:
 //   psi'[s] = cos(th) psi[s] - sg sin(th) psi[t],   psi'[t] = sg sin(th) psi[s] + cos(th) psi[t].
-// Creator and annihilator index sets must be disjoint (excitation operators).
+// Written for excitation operators (disjoint creator and annihilator index sets); generalised doubles that share an
+// index (a^dag_p a^dag_q a_p a_s = -n_p a^dag_q a_s) also satisfy T^2 = 0 and are covered by the same update (pin P9).
 static bool apply_ops(u64 s, const int* cre, int n_cre, const int* ann, int n_ann, u64* t, int* sg) {
     int sign = 1;
     u64 w = s;

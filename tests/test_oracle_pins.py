@@ -332,7 +332,10 @@ def _dense_generator(cre, ann, nq):
     return (T - T.conj().T).toarray()
 
 
-@pytest.mark.parametrize("cre,ann", [((4,), (0,)), ((2, 5), (3, 0)), ((1, 2), (5, 4)), ((2,), (1,))])
+# the last two are generalised doubles with a shared index (tUCCGSD): a^dag_3 a^dag_5 a_3 a_1 = -n_3 a^dag_5 a_1,
+# an X mask of two bits with a number projector attached; creators and annihilators overlap
+@pytest.mark.parametrize("cre,ann", [((4,), (0,)), ((2, 5), (3, 0)), ((1, 2), (5, 4)), ((2,), (1,)),
+                                     ((3, 5), (3, 1)), ((4, 1), (2, 1))])
 def test_p9_fermionic_rotation_vs_dense_expm(cre, ann):
     nq = 6
     Gd = _dense_generator(cre, ann, nq)
