@@ -497,8 +497,9 @@ TRAFFIC_NCU = {
     "q28_hubbard": {"bytes_per_launch": 6.74e8, "kernel": "k_light<0>", "profile": "profiles/r02_q28_k_light_full.md",
                     "note": "Taylor-12 launch mix: 6 odd launches at 487 MB, 5 even at 894 MB, the last (48 D) taken as their mean"},
     "q24": {"bytes_per_launch": None, "kernel": "k_ab<12>", "profile": None},
-    "q32": {"bytes_per_launch": 3.01e10, "kernel": "k_ab<16> (one slab of 1,456 rows; 9 slabs per apply)",
-            "profile": "profiles/r02_q32_q56_launches.md"},
+    "q32": {"bytes_per_launch": 2.96e10, "kernel": "k_ab<16> (one slab of 1,456 rows; 9 slabs per apply)",
+            "profile": "profiles/r02b_q32_k_ab_k_aa_full.md",
+            "note": "dram__bytes_read + dram__bytes_write of two launches: 28.66e9 and 30.58e9"},
     "q56": {"bytes_per_launch": 9.35e10, "kernel": "k_ab<28> (one slab of 2,853 rows; 8 slabs per apply)",
             "profile": "profiles/r02_q32_q56_launches.md"},
 }

@@ -45,7 +45,7 @@
  * Environment (TEST HOOKS, not API; every one is read ONCE, when a plan is built, never on a launch path):
  *   BS_KERNEL=v1|v2inrow   force the v1 sector kernel / keep beta-only groups in-row
  *   BS_NO_LIGHT, BS_LIGHT_THREADS, BS_LIGHT_ORDER, BS_LIGHT_STREAM, BS_LIGHT_COMPACT, BS_LIGHT_SIGN   k_light variants
- *   BS_NO_KRES, BS_NO_HOPSPLIT, BS_KRES_KC, BS_KRES_MIN, BS_KRES_SLAB_MB, BS_KRES_MMA   K-resolved alpha-beta kernel off / chunk / threshold / slab / DFMA form
+ *   BS_NO_KRES, BS_NO_HOPSPLIT, BS_KRES_KC, BS_KRES_MIN, BS_KRES_SLAB_MB, BS_KRES_MMA, BS_KRES_STAGES, BS_KRES_BIG   K-resolved alpha-beta kernel off / chunk / threshold / slab / DFMA form / pipeline buffers (2 | 3) / 16-compute-warp build on or off
  *   BS_NO_K2, BS_K2_MIN, BS_K2_SLAB_MB, BS_K2_MMA, BS_K2_RT, BS_K2_NT, BS_K2_NO_CTILE   K2-resolved same-spin doubles off / threshold / slab / DFMA form / its tile / tensor form's target tiles of 8 / its coupling tiles evaluated in the kernel, not at plan time
  *   BS_ROT_ORBIT=1   orbit cells (k_rot_orbit) for rotation runs instead of row cells (slower at configs[3]; kept as a
  *                    tested alternative); read once per process

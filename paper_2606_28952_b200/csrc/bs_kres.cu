@@ -20,6 +20,7 @@ constexpr u32 kGKeyMask = (1u << 28) - 1;
 constexpr int kMaxDenseStr = 160;     // strings of an absorbed x_b = 0 group (3 n + 1 for a two-body Hamiltonian)
 constexpr int kMaxSegs = 48;          // staged column segments of a K chunk
 constexpr int kProducer = 32;         // threads of the producer warp (the last warp of the block)
+constexpr int kKresBarBytes = 64;     // full[3] + empty[3] mbarriers at the head of k_ab's shared memory (48 bytes used)
 
 // shared-memory layout of one coupling matrix: row s holds G[s][0..NP), padded to a multiple of 8 columns (zero) and to a
 // row stride of 8 k + 4 doubles so that the four rows a half warp reads as an MMA fragment fall on different banks
@@ -119,12 +120,14 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
      i64 row_lo) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint2 sSeg[kMaxSegs];
-    u64* bar = reinterpret_cast<u64*>(smem_raw);   // full[2] (producer + TMA -> compute warps), empty[2] (compute warps -> producer)
+    // NS = 2 or 3 pipeline stages: full[NS] (producer + TMA -> compute warps), empty[NS] (compute warps -> producer)
+    u64* bar = reinterpret_cast<u64*>(smem_raw);
     constexpr int GS = kres_gs(NP), GN = NP * GS, NT = (NP + 7) / 8;
-    double* sG = reinterpret_cast<double*>(smem_raw + 32);                                   // [2][NP][GS]
-    double2* sbuf = reinterpret_cast<double2*>(smem_raw + 32 + 2 * GN * 8);                  // [2][buf_elems]
-    unsigned short* sgo =
-        reinterpret_cast<unsigned short*>(smem_raw + 32 + 2 * GN * 8 + 2 * (size_t)Kd.buf_elems * 16);  // [NP][KC]
+    const int NS = Kd.n_stages;
+    double* sG = reinterpret_cast<double*>(smem_raw + kKresBarBytes);                                        // [NS][NP][GS]
+    double2* sbuf = reinterpret_cast<double2*>(smem_raw + kKresBarBytes + (size_t)NS * GN * 8);              // [NS][buf_elems]
+    unsigned short* sgo = reinterpret_cast<unsigned short*>(smem_raw + kKresBarBytes + (size_t)NS * GN * 8 +
+                                                            (size_t)NS * Kd.buf_elems * 16);               // [NP][KC]
     constexpr int RTW = kres_rtw(NP);
     const int tid = threadIdx.x, KC = Kd.KC, n_cmp = (int)blockDim.x - kProducer;   // K per chunk, compute threads
     const bool producer = tid >= n_cmp;
@@ -141,13 +144,12 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
         for (int g = lane; g < nseg; g += 32) sSeg[g] = __ldg(Kd.segs + (size_t)chunk * Kd.max_segs + g);
     }
     if (tid == n_cmp) {
-        mbar_init(bar, 1);       // full: the producer's arrive.expect_tx; the bulk copies complete the byte count
-        mbar_init(bar + 1, 1);
-        mbar_init(bar + 2, (u32)n_cmp / 32);
-        mbar_init(bar + 3, (u32)n_cmp / 32);
+        for (int b = 0; b < NS; ++b) {
+            mbar_init(bar + b, 1);                     // full: the producer's arrive.expect_tx; the bulk copies complete the byte count
+            mbar_init(bar + NS + b, (u32)n_cmp / 32);  // empty: one arrival per compute warp
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        sbuf[0] = make_double2(0.0, 0.0);             // position 0 of either buffer: the zero amplitude (s in K)
-        sbuf[Kd.buf_elems] = make_double2(0.0, 0.0);
+        for (int b = 0; b < NS; ++b) sbuf[(size_t)b * Kd.buf_elems] = make_double2(0.0, 0.0);   // position 0 of every buffer: the zero amplitude (s in K)
     }
     constexpr int ACCN = MMA ? 4 * RTW * NT : NP;   // MMA: RTW row tiles x NT column tiles x (re, im) fragments of two doubles
     double2 acc[ACCN < NP ? NP : ACCN];
@@ -160,31 +162,39 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
     u32 seg_bytes = 0;   // producer: bytes of one entry's bulk copies
 
     // ---- producer warp -----------------------------------------------------------------------------------------
-    // TMA bulk copies of the chunk's column segments of entry i's source row into buffer i & 1 (lane 0)
-    auto stage_row = [&](int i) {
+    // TMA bulk copies of the chunk's column segments of entry i's source row into buffer b = i mod NS (lane 0)
+    auto stage_row = [&](int i, int b) {
         const u32 src_row = __ldg(reinterpret_cast<const u32*>(Kd.row_ent + e0 + i) + 1);
         const double2* __restrict__ src = psi + (i64)src_row * Db;
-        unsigned char* dst = reinterpret_cast<unsigned char*>(sbuf + (size_t)(i & 1) * Kd.buf_elems + 1);
-        mbar_expect_tx(bar + (i & 1), seg_bytes + (u32)(GN * 8));
+        unsigned char* dst = reinterpret_cast<unsigned char*>(sbuf + (size_t)b * Kd.buf_elems + 1);
+        mbar_expect_tx(bar + b, seg_bytes + (u32)(GN * 8));
         // the entry's coupling matrix, made by k_ab_g for all K chunks of the row
-        tma_bulk_g2s(sG + (i & 1) * GN, Gbuf + (e0 - e_base + i) * GN, (u32)(GN * 8), bar + (i & 1));
+        tma_bulk_g2s(sG + b * GN, Gbuf + (e0 - e_base + i) * GN, (u32)(GN * 8), bar + b);
         for (int g = 0; g < nseg; ++g) {
             const uint2 sg = sSeg[g];
             const unsigned char* sp = reinterpret_cast<const unsigned char*>(src + sg.x);
             const u32 bytes = sg.y * 16u;
-            for (u32 o = 0; o < bytes; o += 32768u) tma_bulk_g2s(dst + o, sp + o, min(32768u, bytes - o), bar + (i & 1));
+            for (u32 o = 0; o < bytes; o += 32768u) tma_bulk_g2s(dst + o, sp + o, min(32768u, bytes - o), bar + b);
             dst += bytes;
         }
     };
     __syncthreads();
     if (producer) {
         // No block barrier in the entry loop: the producer refills buffer b as soon as every compute warp has released
-        // it (empty[b]); a compute warp starts entry i as soon as full[i & 1] completes, whatever the other warps do.
+        // it (empty[b]); a compute warp starts entry i as soon as full[i mod NS] completes, whatever the other warps do.
+        // Entry i uses buffer b = i mod NS for the (i / NS)-th time: its full barrier completes phase i / NS, and the
+        // producer refills it once the empty barrier has completed phase i / NS - 1.  NS = 3 (producer two entries ahead)
+        // was built because 12.5 % of the compute warps' stall samples sit on the full-barrier wait; it changes nothing
+        // (q32 432.7 vs 433.0 ms): that wait is the slack of warps with fewer active orbitals, which a deeper queue cannot
+        // remove.  Two buffers are the default, three a tested hook (BS_KRES_STAGES=3).
         if (lane == 0) {
             for (int g = 0; g < nseg; ++g) seg_bytes += sSeg[g].y * 16u;
+            int b = 0;
+            u32 use = 0;   // i / NS
             for (int i = 0; i < n_ent; ++i) {
-                if (i >= 2) mbar_wait(bar + 2 + (i & 1), (u32)((i >> 1) - 1) & 1u);
-                stage_row(i);
+                if (use > 0) mbar_wait(bar + NS + b, (use - 1) & 1u);
+                stage_row(i, b);
+                if (++b == NS) { b = 0; ++use; }
             }
         }
         return;
@@ -219,10 +229,12 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
             const u32 s_ = 4 * st_ + tq < (u32)n_act ? __fns(act_all, 0, 4 * st_ + tq + 1) : 63u;
             my_orb |= (u64)(s_ & 63u) << (6 * st_);
         }
+        int cb = 0;      // buffer of entry i: i mod NS
+        u32 cuse = 0;    // i / NS
         for (int i = 0; i < n_ent; ++i) {
-            mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
-            const double* __restrict__ G = sG + (i & 1) * GN;
-            const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
+            mbar_wait(bar + cb, cuse & 1u);
+            const double* __restrict__ G = sG + cb * GN;
+            const double2* __restrict__ buf = sbuf + (size_t)cb * Kd.buf_elems;
             for (int ks = 0; ks < n_act; ks += 4) {
                 const u32 s = (u32)(my_orb >> (6 * (ks >> 2))) & 63u;   // this lane's orbital of the step (63: none left)
                 const bool valid = s < 32u;
@@ -250,7 +262,8 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
                     }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar + 2 + (i & 1));   // this warp is done with buffer i & 1
+            if (lane == 0) mbar_arrive(bar + NS + cb);   // this warp is done with the buffer
+            if (++cb == NS) { cb = 0; ++cuse; }
         }
         // C fragment: row g of tile i2 (K = kw + 8 i2), columns 8 j + 2 tq + {0, 1}
 #pragma unroll
@@ -272,10 +285,12 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
     // DFMA form: orbitals walked in ascending order; the gather of the next orbital is issued before the DFMA block of
     // the current one
     const unsigned short* __restrict__ my_go = sgo + tid;
+    int cb = 0;      // buffer of entry i: i mod NS
+    u32 cuse = 0;    // i / NS
     for (int i = 0; i < n_ent; ++i) {
-        mbar_wait(bar + (i & 1), (u32)(i >> 1) & 1u);
-        const double* __restrict__ G = sG + (i & 1) * GN;
-        const double2* __restrict__ buf = sbuf + (size_t)(i & 1) * Kd.buf_elems;
+        mbar_wait(bar + cb, cuse & 1u);
+        const double* __restrict__ G = sG + cb * GN;
+        const double2* __restrict__ buf = sbuf + (size_t)cb * Kd.buf_elems;
         u32 act = act_all;
         int s = __ffs((int)act) - 1;
         act &= act - 1;
@@ -301,7 +316,8 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
             b = bn;
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar + 2 + (i & 1));   // this warp is done with buffer i & 1
+        if (lane == 0) mbar_arrive(bar + NS + cb);   // this warp is done with the buffer
+        if (++cb == NS) { cb = 0; ++cuse; }
     }
     double2* __restrict__ out = S + ((i64)blockIdx.x * Kd.n) * Kd.DKp + (i64)chunk * KC + tid;
 #pragma unroll
@@ -313,13 +329,25 @@ k_ab(const KresDev Kd, const double2* __restrict__ psi, const double* __restrict
     }
 }
 
-// compute threads + the producer warp fill whole groups of 4 warps (one per SM sub-partition): 512 threads at <= 128
-// registers for up to 16 orbitals, 256 threads at <= 255 registers above
-constexpr int kres_kcmax(int NP) { return NP <= 16 ? 480 : 224; }
+// K per chunk.  DFMA form (one thread per K): compute threads + the producer warp fill whole groups of 4 warps, 512 threads
+// at <= 128 registers for up to 16 orbitals, 256 threads at <= 255 registers above.  Tensor form (8 RTW K per warp): 16
+// COMPUTE warps, four per SM sub-partition, plus the producer warp (544 threads at <= 120 registers).  With 480 / 224 K the
+// tensor form ran 15 / 14 compute warps: the busiest sub-partition carried 12 - 15 % more DMMA work than the mean, which is
+// the idle fifth of the tensor pipe that ncu showed (profiles/r02b_q32_k_ab_k_aa_full.md).  The register file is per
+// sub-partition (16 K registers): the sub-partition that also hosts the producer warp holds five warps, so the 544-thread
+// builds are capped at 96 registers.  Above 16 orbitals (two row tiles per warp) that costs at most 16 bytes of spills
+// and the balance wins 8 % (q56 1,107 -> 1,015 ms); up to 16 orbitals (four row tiles, 117 registers) it costs 52 bytes of
+// spills: worth it only for sectors with many chunks (q32 438.5 -> 431.8 ms), not for small ones (q24 1.233 -> 1.277 ms),
+// which keep the 480 build (`big` = false).
+constexpr int kres_kcmax(int NP, bool mma, bool big) {
+    return mma ? (NP <= 16 ? (big ? 512 : 480) : 256) : (NP <= 16 ? 480 : 224);
+}
 
 template <int NP>
 cudaError_t kab_launch(const bs_kres* K, const double2* psi, i64 lo, i64 hi, cudaStream_t st, bool set_attr) {
-    auto k = K->mma ? k_ab<NP, kres_kcmax(NP), true> : k_ab<NP, kres_kcmax(NP), false>;
+    auto k = !K->mma ? k_ab<NP, kres_kcmax(NP, false, false), false>
+                     : (K->kc_max == kres_kcmax(NP, true, true) ? k_ab<NP, kres_kcmax(NP, true, true), true>
+                                                                : k_ab<NP, kres_kcmax(NP, true, false), true>);
     // the ceiling is per kernel and shared by all plans: the opt-in maximum minus the kernel's static shared memory
     if (set_attr) return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024);
     dim3 grid((unsigned)(hi - lo), (unsigned)K->n_chunks);
@@ -463,8 +491,15 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
     auto col_of = [&](u32 w) {
         return (i64)(std::lower_bound(S->h_sb.begin(), S->h_sb.end(), (u64)w) - S->h_sb.begin());
     };
-    const int kc_max = kres_kcmax(NP);   // register budget of k_ab<NP>
-    int KC = (int)std::min<i64>(kc_max, (DK + 31) / 32 * 32);
+    K->mma = getenv("BS_KRES_MMA") ? atoi(getenv("BS_KRES_MMA")) != 0 : true;   // test hook: 0 = DFMA form
+    // the build of k_ab (register budget): the 16-compute-warp build for sectors with at least 8 chunks of it
+    bool big = (DK + kres_kcmax(NP, K->mma, true) - 1) / kres_kcmax(NP, K->mma, true) >= 8;
+    if (const char* e = getenv("BS_KRES_BIG")) big = atoi(e) != 0;   // test hook: force either build
+    const int kc_max = kres_kcmax(NP, K->mma, big);
+    K->kc_max = kc_max;
+    // chunks of equal size: K strings split evenly over the fewest chunks (q24: 792 K in 2 chunks of 416, not 480 + 312)
+    const i64 n_min = (DK + kc_max - 1) / kc_max;
+    int KC = (int)std::min<i64>(kc_max, ((DK + n_min - 1) / n_min + 31) / 32 * 32);
     if (const char* e = getenv("BS_KRES_KC")) KC = std::max(32, std::min(kc_max, atoi(e) / 32 * 32));
     const size_t smem_max = 227 * 1024 - 1024;
     std::vector<uint2> segs;
@@ -517,9 +552,15 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
                     goff[((size_t)c * NP + s) * KC + (k - (i64)c * KC)] = (unsigned short)(base[g] + (col - sg[g].x));
                 }
         }
-        const size_t smem = 32 + 2 * (size_t)NP * kres_gs(NP) * 8 + 2 * (size_t)buf_elems * 16 + (size_t)NP * KC * 2;
+        auto smem_for = [&](int ns) {
+            return (size_t)kKresBarBytes + (size_t)ns * NP * kres_gs(NP) * 8 + (size_t)ns * buf_elems * 16 + (size_t)NP * KC * 2;
+        };
+        const size_t smem = smem_for(2);   // the chunk size is chosen for two buffers, as before
         if (smem <= smem_max && buf_elems <= 65535) {
-            K->smem = smem;
+            // two buffers; BS_KRES_STAGES=3 (test hook) takes a third when it fits at this chunk size: no measured gain
+            K->n_stages = 2;
+            if (const char* e = getenv("BS_KRES_STAGES")) K->n_stages = (atoi(e) >= 3 && smem_for(3) <= smem_max) ? 3 : 2;
+            K->smem = smem_for(K->n_stages);
             segs.assign((size_t)n_chunks * max_segs, make_uint2(0u, 0u));
             segcnt.resize(n_chunks);
             for (int c = 0; c < n_chunks; ++c) {
@@ -530,7 +571,6 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
         }
     }
     K->KC = KC;
-    K->mma = getenv("BS_KRES_MMA") ? atoi(getenv("BS_KRES_MMA")) != 0 : true;   // test hook: 0 = DFMA form
     K->n_chunks = n_chunks;
     K->max_segs = max_segs;
     K->buf_elems = buf_elems;
@@ -600,6 +640,7 @@ int bs_kres_build(std::vector<HostGroup>& groups, bs_sector* S, cudaStream_t st,
     d.n = n;
     d.Nb = Nb;
     d.buf_elems = buf_elems;
+    d.n_stages = K->n_stages;
     d.Db = S->Db;
     d.DKp = K->DKp;
     d.inv_nb = 1.0 / (double)Nb;

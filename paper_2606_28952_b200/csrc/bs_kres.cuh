@@ -46,6 +46,7 @@ struct KresDev {
     const uint2* segs;           // [n_chunks][max_segs] {first column, length} of the staged column segments
     const int* seg_cnt;          // [n_chunks]
     int max_segs, KC, n_chunks, n, Nb, buf_elems;
+    int n_stages;   // shared-memory buffers of k_ab's producer / consumer pipeline: 3 when they fit, else 2
     i64 Db, DKp;
     double inv_nb;
 };
@@ -60,7 +61,8 @@ struct KresComb {
 
 struct bs_kres {
     bs_rowplan* rp = nullptr;
-    int n = 0, NP = 0, Nb = 0, KC = 0, n_chunks = 0, max_segs = 0, buf_elems = 0;
+    int n = 0, NP = 0, Nb = 0, KC = 0, n_chunks = 0, max_segs = 0, buf_elems = 0, n_stages = 2;
+    int kc_max = 0;   // the KCMAX instantiation of k_ab this plan launches (its launch bound fixes the register budget)
     i64 DK = 0, DKp = 0, slab_rows = 0;
     size_t smem = 0;
     bool mma = true;             // contraction on the FP64 tensor instruction (else DFMA)

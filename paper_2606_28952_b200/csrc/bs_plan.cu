@@ -407,10 +407,10 @@ extern "C" int bs_plan_describe(bs_op_t op, bs_sector_t s, char* buf, int64_t n,
         if (P->kres && w > 0 && w < n) {
             const bs_kres* K = P->kres;
             w += snprintf(buf + w, (size_t)(n - w),
-                          " kres{xa=%d keys=%lld DK=%lld KC=%d chunks=%d NP=%d smem=%zu staged_rows=%.2f max_segs=%d slab_rows=%lld "
+                          " kres{xa=%d keys=%lld DK=%lld KC=%d chunks=%d NP=%d smem=%zu stages=%d staged_rows=%.2f max_segs=%d slab_rows=%lld "
                           "scratch_MB=%.0f}",
                           K->rp->n_xa, (long long)K->rp->n_keys, (long long)K->DK, K->KC, K->n_chunks, K->NP, K->smem,
-                          K->staged_rows, K->max_segs, (long long)K->slab_rows,
+                          K->n_stages, K->staged_rows, K->max_segs, (long long)K->slab_rows,
                           (double)K->slab_rows * K->n * K->DKp * 16.0 / 1048576.0);
         }
         for (const bs_k2* K2 : {P->k2_main, P->k2_t})

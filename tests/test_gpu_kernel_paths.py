@@ -108,6 +108,10 @@ print('PATH OK')
     ({"BS_K2_SLAB_MB": "1", "BS_K2_MIN": "1", "BS_NO_HOPSPLIT": "1"}, "kres{"),              # several column slabs of the K2 scratch
     ({"BS_KRES_KC": "64", "BS_KRES_SLAB_MB": "2", "BS_K2_MMA": "0"}, "kres{"),   # more K chunks, several scratch slabs, DFMA k_aa
     ({"BS_KRES_KC": "32", "BS_KRES_MIN": "1", "BS_KRES_MMA": "0"}, "kres{"),   # DFMA form of the K-resolved contraction
+    ({"BS_KRES_STAGES": "3", "BS_KRES_MIN": "1"}, "kres{"),                    # three pipeline buffers in k_ab (default: two)
+    ({"BS_KRES_STAGES": "3", "BS_KRES_KC": "64", "BS_KRES_MMA": "0"}, "kres{"),
+    ({"BS_KRES_BIG": "1", "BS_KRES_MIN": "1"}, "kres{"),                       # the 16-compute-warp (96-register) build of k_ab
+    ({"BS_KRES_BIG": "1", "BS_KRES_KC": "96", "BS_KRES_STAGES": "3"}, "kres{"),
     ({"BS_K2_NT": "2", "BS_K2_MIN": "1"}, "kres{"),   # k_aa_mma target tiles of 16 / 24 / 32: <2, 4, 1>, <3, 2, 3>, <4, 2, 3>
     ({"BS_K2_NT": "3", "BS_K2_MIN": "1", "BS_K2_SLAB_MB": "1"}, "kres{"),
     ({"BS_K2_NT": "4", "BS_K2_MIN": "1"}, "kres{"),
