@@ -9,6 +9,7 @@
 //   psi'[u] = cos(theta r) psi[u] - sin(theta r)/r conj(F(t)) psi[t].
 // Routing (pairing) and phase accumulation are computed once per pair and group.
 // The pair is owned by the thread of its smaller index, so the update is in place and race free.
+#include <cooperative_groups.h>
 #include <algorithm>
 
 #include "bs_internal.cuh"
@@ -261,6 +262,58 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
             psi[(i64)row0 * Db + c] = s0[c];
             if (R == 2) psi[(i64)row1 * Db + c] = s1[c];
         }
+}
+
+// Row-pair cells whose two rows do not fit ONE block's shared memory (D_beta = 12,870 at configs[3]: 2 x 206 KB) but
+// whose single row does: a thread-block cluster of two, one row per block, the partner amplitude of every pair reached
+// through distributed shared memory (a generic pointer from map_shared_rank).  Same run, same pair lists and the same
+// arithmetic per pair as k_rot_cell_rows<2, false>; the pair list is split over the 2 x 512 threads of the cluster and the
+// barrier between generators is the cluster's.  Replaces the in-place (L2) form there, which moves 64 bytes per pair
+// through L2 for every generator.
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(512)
+k_rot_cluster_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
+                   const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
+                   const double* __restrict__ thetas, const double2* __restrict__ sc, const uint2* __restrict__ cpairs,
+                   const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
+    namespace cg = cooperative_groups;
+    extern __shared__ __align__(16) unsigned char smem_cell[];
+    __shared__ GenChunk G;
+    cg::cluster_group cluster = cg::this_cluster();
+    const unsigned rank = cluster.block_rank();            // 0 holds row0, 1 holds row1
+    const u32 Db = (u32)B.D;
+    const uint2 pr = pairs[blockIdx.x >> 1];
+    const u32 my_row = rank ? pr.y : pr.x;
+    double2* mine = reinterpret_cast<double2*>(smem_cell);
+    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) mine[c] = psi[(i64)my_row * Db + c];
+    double2* s0 = rank == 0 ? mine : cluster.map_shared_rank(mine, 0);
+    double2* s1 = rank == 1 ? mine : cluster.map_shared_rank(mine, 1);
+    const u32 ta = A.str[pr.x];
+    const u32 tid2 = rank * blockDim.x + threadIdx.x, stride2 = 2 * blockDim.x;
+    cluster.sync();   // both rows are in shared memory before anyone reaches across
+    for (i64 j = j0; j < j1;) {
+        __syncthreads();  // this block's previous chunk fully consumed (G is per block)
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        __syncthreads();
+        for (int i = threadIdx.x; i < min(G.k0[n], kStrChunk); i += blockDim.x) {
+            const u64 zz = G.z[i];
+            const u32 par = (u32)__popc((u32)(zz & ((u64(1) << n_orb) - 1)) & ta) & 1u;
+            G.w[i] = make_double2(flipd(G.w[i].x, par), flipd(G.w[i].y, par));
+            G.z[i] = zz >> n_orb;
+        }
+        __syncthreads();
+        for (int g = 0; g < n; ++g) {
+            const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
+            const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
+            for (i64 p = p0 + tid2; p < p1; p += stride2) {
+                const uint2 cp = __ldg(cpairs + p);
+                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, B.str[cp.x]), G.th[g], G.sc[g]);
+            }
+            cluster.sync();   // the next generator may pair these amplitudes with others, from either block
+        }
+        j += n;
+    }
+    // the last cluster.sync() above ordered every remote write before this read of the block's own row
+    for (u32 c = threadIdx.x; c < Db; c += blockDim.x) psi[(i64)my_row * Db + c] = mine[c];
 }
 
 // cells = CC consecutive columns x all rows (x_b = 0 for every generator of the run); GLOBAL as above (in place, L2)
@@ -682,6 +735,9 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     // BS_ROT_ORBIT=1 (test hook): orbit cells (k_rot_orbit) for common-x_a runs at any sector size.  Not the default:
     // measured slower than the in-place cells at configs[3] (1.79 s vs 1.32 s for the UCCSD list)
     static const int orbit_mode = getenv("BS_ROT_ORBIT") ? atoi(getenv("BS_ROT_ORBIT")) : 0;
+    // row pairs too large for one block's shared memory in a cluster of two blocks (k_rot_cluster_rows): opt-in
+    // 1: where the pair does not fit one block; 2 (test hook): every row-pair run whose single row fits
+    static const int cluster_rows = getenv("BS_ROT_CLUSTER") ? atoi(getenv("BS_ROT_CLUSTER")) : 0;
     const bool batching = RR && RR->coff.back() > 0 && !env_per_launch;
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
@@ -729,7 +785,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 const uint2* pr = RR->d_pairs.p + RR->off[j];
                 if (n_cells == 0) {
                     launched = true;  // x_a never valid in this sector: identity
-                } else if (smem <= smem_cap && !in_place && orbit_mode != 1) {
+                } else if (smem <= smem_cap && !in_place && orbit_mode != 1 && !(R == 2 && cluster_rows == 2)) {
                     if (R == 2) {
                         BS_ROT_SMEM((k_rot_cell_rows<2, false>))
                         k_rot_cell_rows<2, false><<<(unsigned)n_cells, 512, smem, st>>>(BS_ROT_ARGS_ROWS);
@@ -737,6 +793,15 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                         BS_ROT_SMEM((k_rot_cell_rows<1, false>))
                         k_rot_cell_rows<1, false><<<(unsigned)n_cells, 256, smem, st>>>(BS_ROT_ARGS_ROWS);
                     }
+                    BS_COUNT_LAUNCH(1);
+                    launched = true;
+                } else if (R == 2 && cluster_rows && !in_place && orbit_mode != 1 &&
+                           (size_t)s->Db * 16 + sizeof(GenChunk) + 1024 <= (size_t)227 * 1024) {
+                    // one row per block of a two-block cluster (the pair does not fit one block, a single row does)
+                    static const cudaError_t e_attr = cudaFuncSetAttribute(
+                        k_rot_cluster_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024 - (int)sizeof(GenChunk));
+                    BS_CUDA(e_attr);
+                    k_rot_cluster_rows<<<(unsigned)(2 * n_cells), 512, (size_t)s->Db * 16, st>>>(BS_ROT_ARGS_ROWS);
                     BS_COUNT_LAUNCH(1);
                     launched = true;
                 } else if (!RR->orbit_subs.empty() && orbit_mode == 1 && !in_place) {
