@@ -49,6 +49,9 @@
  *   BS_NO_K2, BS_K2_MIN, BS_K2_SLAB_MB, BS_K2_MMA, BS_K2_RT, BS_K2_NT, BS_K2_NO_CTILE   K2-resolved same-spin doubles off / threshold / slab / DFMA form / its tile / tensor form's target tiles of 8 / its coupling tiles evaluated in the kernel, not at plan time
  *   BS_ROT_ORBIT=1   orbit cells (k_rot_orbit) for rotation runs instead of row cells (slower at configs[3]; kept as a
  *                    tested alternative); read once per process
+ *   BS_ROT_CSTR=0 | 1   row-cell rotation kernels read a column's string from the sector's table (0) or from a copy kept with
+ *                    the pair list (1); default: the copy where amplitudes come through L2 (in place, cluster), the table
+ *                    where the cell is in shared memory; read once per process
  *   BS_ROT_CLUSTER=1 | 2   row-pair runs on a thread-block cluster of two, one row per block, partners through distributed
  *                    shared memory (k_rot_cluster_rows): 1 = where the pair exceeds one block's shared memory, 2 = every
  *                    row-pair run (test hook).  Slower than the in-place form at configs[3] (1.62 s vs 1.32 s); kept as a

@@ -87,6 +87,8 @@ struct bs_op {
         DevBuf<uint2> d_pairs;  // {row, partner row}
         std::vector<i64> coff;  // [G + 1]
         DevBuf<uint2> d_cpairs; // per generator the valid {column, partner column} pairs (x_a = 0: owner side only)
+        DevBuf<u32> d_cstr;     // the column spin's string of every d_cpairs entry's first column: read WITH the pair, so the
+                                // phase sum does not wait for a second dependent look-up (B.str[column])
         DevBuf<i64> d_off, d_coff;  // device copies of off / coff
         std::vector<i64> roff;  // [G + 1] z-reduced strings of every generator for this sector (exact on valid targets)
         DevBuf<u64> d_rz;

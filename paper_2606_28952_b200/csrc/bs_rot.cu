@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(R == 2 ? 512 : 256)
 k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
                 const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
                 const double* __restrict__ thetas, const double2* __restrict__ sc, const uint2* __restrict__ cpairs,
-                const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
+                const u32* __restrict__ cstr, const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
     const u32 Db = (u32)B.D;
@@ -251,7 +251,8 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
             const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
             for (i64 p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
                 const uint2 cp = __ldg(cpairs + p);
-                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, B.str[cp.x]), G.th[g], G.sc[g]);
+                const u32 tb = cstr ? __ldg(cstr + p) : B.str[cp.x];   // the list copy: no dependent look-up
+                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, tb), G.th[g], G.sc[g]);
             }
             __syncthreads();
         }
@@ -274,7 +275,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(512)
 k_rot_cluster_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs, const u64* __restrict__ xg,
                    const i64* __restrict__ offs, const u64* __restrict__ z, const double2* __restrict__ w,
                    const double* __restrict__ thetas, const double2* __restrict__ sc, const uint2* __restrict__ cpairs,
-                   const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
+                   const u32* __restrict__ cstr, const i64* __restrict__ coff, i64 j0, i64 j1, double2* __restrict__ psi) {
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char smem_cell[];
     __shared__ GenChunk G;
@@ -306,7 +307,8 @@ k_rot_cluster_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pa
             const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
             for (i64 p = p0 + tid2; p < p1; p += stride2) {
                 const uint2 cp = __ldg(cpairs + p);
-                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, B.str[cp.x]), G.th[g], G.sc[g]);
+                const u32 tb = cstr ? __ldg(cstr + p) : B.str[cp.x];
+                rotate_smem(s0[cp.x], s1[cp.y], phase_sum_b(G, k0, k1, tb), G.th[g], G.sc[g]);
             }
             cluster.sync();   // the next generator may pair these amplitudes with others, from either block
         }
@@ -544,6 +546,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
             // column pairs per generator (independent of the row): valid columns and their partners; for x_a = 0 the
             // pair lives in one row and is listed once (smaller column first)
             std::vector<uint2> cpairs;
+            std::vector<u32> cstr;
             RR->coff.assign(n_rot + 1, 0);
             if ((double)n_rot * (double)s->Db <= 5e8) {
                 for (i64 j = 0; j < n_rot; ++j) {
@@ -555,6 +558,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                         const i64 uc = xb ? (i64)(std::lower_bound(s->h_sb.begin(), s->h_sb.end(), tb ^ xb) - s->h_sb.begin()) : c;
                         if (xa == 0 && uc <= c) continue;
                         cpairs.push_back(make_uint2((u32)c, (u32)uc));
+                        cstr.push_back((u32)tb);
                     }
                     RR->coff[j + 1] = (i64)cpairs.size();
                 }
@@ -687,6 +691,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
             if (e == cudaSuccess) e = RR->d_rw.upload(rw, st);
             if (e == cudaSuccess) e = RR->d_roff.upload(RR->roff, st);
             if (e == cudaSuccess) e = RR->d_cpairs.upload(cpairs, st);
+            if (e == cudaSuccess) e = RR->d_cstr.upload(cstr, st);
             if (e == cudaSuccess) e = RR->d_off.upload(RR->off, st);
             if (e == cudaSuccess) e = RR->d_coff.upload(RR->coff, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -738,6 +743,8 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
     // row pairs too large for one block's shared memory in a cluster of two blocks (k_rot_cluster_rows): opt-in
     // 1: where the pair does not fit one block; 2 (test hook): every row-pair run whose single row fits
     static const int cluster_rows = getenv("BS_ROT_CLUSTER") ? atoi(getenv("BS_ROT_CLUSTER")) : 0;
+    // column strings read from the pair list (1) or from the sector's string table (0); test hook, default below
+    static const int cstr_mode = getenv("BS_ROT_CSTR") ? atoi(getenv("BS_ROT_CSTR")) : -1;
     const bool batching = RR && RR->coff.back() > 0 && !env_per_launch;
     {
         const size_t smem_cap = 190 * 1024;  // + the static generator chunk (7.5 KB)
@@ -770,7 +777,7 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
             for (i64 q = j; q < e && kind; ++q)
                 if (RR->roff[q + 1] - RR->roff[q] > 256) kind = 0;  // kStrChunk
 #define BS_ROT_ARGS_ROWS s->ta, s->tb, s->n_orb, pr, gen->d_xg.p, RR->d_roff.p, RR->d_rz.p, RR->d_rw.p, RR->d_th.p, RR->d_sc.p, \
-                         RR->d_cpairs.p, RR->d_coff.p, j, e, psi
+                         RR->d_cpairs.p, cstr_arg, RR->d_coff.p, j, e, psi
 #define BS_ROT_ARGS_COLS s->ta, s->tb, s->n_orb, gen->d_xg.p, RR->d_roff.p, RR->d_rz.p, RR->d_rw.p, RR->d_th.p, RR->d_sc.p, \
                          RR->d_pairs.p, RR->d_off.p, j, e, psi
 #define BS_ROT_SMEM(K)                                                                                              \
@@ -783,6 +790,11 @@ extern "C" int bs_apply_pauli_rotations(bs_op_t gen, bs_sector_t s, const double
                 const size_t smem = (size_t)R * s->Db * 16;
                 const i64 n_cells = xa0 ? RR->off[j + 1] - RR->off[j] : s->Da;
                 const uint2* pr = RR->d_pairs.p + RR->off[j];
+                // column strings: from the pair list where the amplitudes come through L2 (in place, cluster: one dependent
+                // look-up fewer, q32 1,323 -> 1,260 ms), from the sector's table (hot in L1) where the cell is in shared
+                // memory; BS_ROT_CSTR = 0 | 1 forces either
+                const bool cells_in_smem = smem <= smem_cap && !in_place && orbit_mode != 1 && !(R == 2 && cluster_rows == 2);
+                const u32* cstr_arg = (cstr_mode >= 0 ? cstr_mode != 0 : !cells_in_smem) ? RR->d_cstr.p : nullptr;
                 if (n_cells == 0) {
                     launched = true;  // x_a never valid in this sector: identity
                 } else if (smem <= smem_cap && !in_place && orbit_mode != 1 && !(R == 2 && cluster_rows == 2)) {

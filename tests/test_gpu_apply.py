@@ -346,7 +346,8 @@ def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
     # BS_ROT_CLUSTER=2: every row-pair run on a cluster of two blocks, one row each, partners through distributed shared
     # memory (opt-in with =1 for sectors whose row pair exceeds one block's shared memory)
     for key, env in (("cells", {}), ("per_launch", {"BS_ROT_PER_LAUNCH": "1"}), ("in_place", {"BS_ROT_IN_PLACE": "1"}),
-                     ("orbit", {"BS_ROT_ORBIT": "1"}), ("cluster", {"BS_ROT_CLUSTER": "2"})):
+                     ("orbit", {"BS_ROT_ORBIT": "1"}), ("cluster", {"BS_ROT_CLUSTER": "2"}),
+                     ("cstr", {"BS_ROT_CSTR": "1"}), ("in_place_table", {"BS_ROT_IN_PLACE": "1", "BS_ROT_CSTR": "0"})):
         r = subprocess.run([sys.executable, "-c", code, root], env=dict(os.environ, **env), capture_output=True,
                            text=True, timeout=600)
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
@@ -354,7 +355,7 @@ def test_rotations_shuffled_order_and_per_launch_path(bs, orc):
     assert counts["per_launch"] > 3 * counts["cells"]      # batching really reduces the launch count
     assert counts["in_place"] == counts["cells"]
     assert counts["cells"] <= counts["orbit"] < counts["per_launch"]
-    assert counts["cluster"] == counts["cells"]
+    assert counts["cluster"] == counts["cells"] == counts["cstr"] == counts["in_place_table"]
 
 
 def test_apply_and_rotations_are_bit_reproducible(bs):
