@@ -157,6 +157,8 @@ struct GenChunk {
     double th[kGenChunk];
     u64 x[kGenChunk];
     int k0[kGenChunk + 1];  // string offsets relative to the chunk
+    i64 p0[kGenChunk + 1];  // bounds of every generator's pair list (coff / roff): staged with the headers, so that a
+                            // generator's loop does not start with a dependent global look-up
     int n;                  // generators in the chunk
 };
 
@@ -164,7 +166,7 @@ struct GenChunk {
 __device__ __forceinline__ int load_chunk(GenChunk& G, i64 j, i64 j1, const u64* __restrict__ xg,
                                           const i64* __restrict__ offs, const u64* __restrict__ z,
                                           const double2* __restrict__ w, const double* __restrict__ thetas,
-                                          const double2* __restrict__ sc) {
+                                          const double2* __restrict__ sc, const i64* __restrict__ pair_off) {
     const i64 base = offs[j];
     int n = (int)min((i64)kGenChunk, j1 - j);
     while (n > 1 && offs[j + n] - base > kStrChunk) --n;  // uniform
@@ -174,7 +176,10 @@ __device__ __forceinline__ int load_chunk(GenChunk& G, i64 j, i64 j1, const u64*
         G.th[i] = thetas[j + i];
         G.sc[i] = sc[j + i];
     }
-    for (int i = threadIdx.x; i <= n; i += blockDim.x) G.k0[i] = (int)(offs[j + i] - base);
+    for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+        G.k0[i] = (int)(offs[j + i] - base);
+        G.p0[i] = pair_off[j + i];
+    }
     for (int i = threadIdx.x; i < ns; i += blockDim.x) {
         G.z[i] = z[base + i];
         G.w[i] = w[base + i];
@@ -233,7 +238,7 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
     const u32 ta = A.str[row0];
     for (i64 j = j0; j < j1;) {
         __syncthreads();  // previous chunk fully consumed (and the rows are loaded)
-        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc, coff);
         __syncthreads();
         // fold the alpha half of every sign into the weights (t_a is fixed for the block): the per-column phase
         // sum is then one 32-bit AND + POPC per string
@@ -248,7 +253,7 @@ k_rot_cell_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pairs
             // the valid (column, partner column) pairs of the generator's beta mask were listed at plan time (they do
             // not depend on the row): no validity test, no rank lookup, no idle lanes
             const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
-            const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
+            const i64 p0 = G.p0[g], p1 = G.p0[g + 1];
             for (i64 p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
                 const uint2 cp = __ldg(cpairs + p);
                 const u32 tb = cstr ? __ldg(cstr + p) : B.str[cp.x];   // the list copy: no dependent look-up
@@ -293,7 +298,7 @@ k_rot_cluster_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pa
     cluster.sync();   // both rows are in shared memory before anyone reaches across
     for (i64 j = j0; j < j1;) {
         __syncthreads();  // this block's previous chunk fully consumed (G is per block)
-        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc, coff);
         __syncthreads();
         for (int i = threadIdx.x; i < min(G.k0[n], kStrChunk); i += blockDim.x) {
             const u64 zz = G.z[i];
@@ -304,7 +309,7 @@ k_rot_cluster_rows(SpinTab A, SpinTab B, int n_orb, const uint2* __restrict__ pa
         __syncthreads();
         for (int g = 0; g < n; ++g) {
             const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
-            const i64 p0 = coff[j + g], p1 = coff[j + g + 1];
+            const i64 p0 = G.p0[g], p1 = G.p0[g + 1];
             for (i64 p = p0 + tid2; p < p1; p += stride2) {
                 const uint2 cp = __ldg(cpairs + p);
                 const u32 tb = cstr ? __ldg(cstr + p) : B.str[cp.x];
@@ -340,13 +345,13 @@ k_rot_cell_cols(SpinTab A, SpinTab B, int n_orb, const u64* __restrict__ xg, con
         }
     for (i64 j = j0; j < j1;) {
         __syncthreads();
-        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc);
+        const int n = load_chunk(G, j, j1, xg, offs, z, w, thetas, sc, roff);
         __syncthreads();
         for (int g = 0; g < n; ++g) {
             // owner (row, partner row) pairs of the generator were listed at plan time: one work item per (pair, column)
             const int k0 = G.k0[g], k1 = min(G.k0[g + 1], kStrChunk);
-            const i64 p0 = roff[j + g];
-            const u32 np = (u32)(roff[j + g + 1] - p0);
+            const i64 p0 = G.p0[g];
+            const u32 np = (u32)(G.p0[g + 1] - p0);
             for (u32 i = threadIdx.x; i < np * CC; i += blockDim.x) {
                 const u32 q = i / CC, c = i - q * CC;
                 if (c >= ncol) continue;
