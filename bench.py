@@ -500,8 +500,8 @@ TRAFFIC_NCU = {
     "q32": {"bytes_per_launch": 2.96e10, "kernel": "k_ab<16> (one slab of 1,456 rows; 9 slabs per apply)",
             "profile": "profiles/r02b_q32_k_ab_k_aa_full.md",
             "note": "dram__bytes_read + dram__bytes_write of two launches: 28.66e9 and 30.58e9"},
-    "q56": {"bytes_per_launch": 9.35e10, "kernel": "k_ab<28> (one slab of 2,853 rows; 8 slabs per apply)",
-            "profile": "profiles/r02_q32_q56_launches.md"},
+    "q56": {"bytes_per_launch": 9.74e10, "kernel": "k_ab<28> (one slab of 2,880 rows; 8 slabs per apply)",
+            "profile": "profiles/r02c_q56_k_ab_full.md"},
 }
 
 
